@@ -1,0 +1,172 @@
+/* include/blest.h -- C ABI of the B200-native BLEST hot path (arXiv 2606.05081).
+ *
+ * Level-synchronous BFS as an iterated bit-level SpMSpV  x(k+1) = (A x(k)) AND NOT v(k)
+ * (Eq. 1) over a Binarized Virtual Slice Set (BVSS), plus the bit-packed
+ * multi-source variant (Alg. 5) and closeness centrality.
+ * Every step of the path runs in hand-written sm_100a CUDA kernels inside this library; the Python
+ * binding (paper_2606_05081_b200/binding.py) only marshals arguments.
+ *
+ * Conventions
+ *  - All functions return an int status: BLEST_OK (0) or a negative BLEST_E* code.  Nothing throws or aborts.
+ *    blest_strerror() names a status; blest_last_cuda_error() returns the cudaError_t behind BLEST_ECUDA.
+ *  - The caller always speaks ORIGINAL vertex ids, whatever reordering blest_build applied inside.
+ *  - Ownership: the library never keeps or frees caller memory.  blest_build copies what it needs; outputs
+ *    are caller-allocated.  Output pointers may be DEVICE pointers (e.g. a torch tensor's data_ptr()) or
+ *    HOST pointers (pinned or pageable): the library detects which with cudaPointerGetAttributes and, for
+ *    host outputs, copies device->host on `cuda_stream` inside the call.
+ *  - Asynchrony: traversal calls enqueue on `cuda_stream` (a cudaStream_t cast to void*, NULL = legacy
+ *    default stream) and return; results are valid once the stream is synchronised.  One handle owns one
+ *    workspace: calls on the same handle must be stream-ordered.  Host `srcs` arrays are consumed before return.
+ *  - Graph precondition: symmetric (undirected) CSR, rows sorted ascending, column ids < n,
+ *    rowptr[0] = 0, rowptr[n] = nnz < 2^32, 1 <= n <= 2^29.  Unsorted rows are always detected
+ *    (BLEST_EUNSORTED); symmetry and ranges are checked only when options.validate != 0.
+ */
+#ifndef BLEST_H
+#define BLEST_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct blest_graph *blest_handle_t; /* opaque; owns device BVSS, device CSR, perm/iperm, workspace */
+
+enum {
+  BLEST_OK = 0,
+  BLEST_EINVAL = -1,       /* NULL pointer, src >= n, k = 0, bad option value */
+  BLEST_ERANGE = -2,       /* n = 0, n > 2^29, nnz >= 2^32, slice count overflow */
+  BLEST_EUNSORTED = -3,    /* a CSR row is not sorted ascending */
+  BLEST_ENOTSYM = -4,      /* (validate only) structure is not symmetric / column id out of range */
+  BLEST_ENOMEM = -5,       /* host or device allocation failed */
+  BLEST_ECUDA = -6,        /* a CUDA call failed; see blest_last_cuda_error() */
+  BLEST_EUNSUPPORTED = -7, /* no sm_100 device / cooperative launch unavailable */
+  BLEST_EOVERFLOW = -8     /* internal work queue overflow (should not happen; reported, never silent) */
+};
+
+/* Input graph ("CSC of A"; symmetric here, so one CSR serves as A, A^T and Alg. 4's CSR(G^T)). */
+typedef struct {
+  uint32_t n;             /* vertices */
+  uint64_t nnz;           /* directed entries = 2 * undirected edges */
+  const uint32_t *rowptr; /* n+1 entries */
+  const uint32_t *colidx; /* nnz entries */
+  int on_device;          /* 0: host pointers, 1: device pointers (copied to the host for the host builder) */
+} blest_csr_t;
+
+/* Options.  Zero-initialised == defaults.  reorder/builder/validate are used by blest_build only; the rest
+ * can be changed later with blest_configure (so that every path can be forced on one handle: the
+ * policy-independence tests and the ablation axes of PAPER.md Tables 4/6). */
+typedef struct {
+  int reorder;     /* 0 none | 1 RCM | 2 degree-descending (BASELINE.json config 4) */
+  int builder;     /* 0 host (OpenMP) | 1 device (BVSS built by CUDA kernels) */
+  int validate;    /* 0 | 1: O(nnz log d) symmetry + range check */
+  int kernel;      /* 0 auto by U_div | 1 eager (Alg. 2) | 2 lazy two-stage (Alg. 3) */
+  int switching;   /* 0 auto (per-level cost model; Eq. 6 analogue) | 1 off: slice path only |
+                      2 force bottom-up CUDA-core (Alg. 4) on every level >= 2 |
+                      3 force top-down CUDA-core (CSR edge chunks) | 4 force slice path */
+  int contraction; /* 0 auto | 1 ALU (AND + per-byte test) | 2 mma.sync m8n8k128 b1 and.popc (paper layout, Fig. 3) |
+                      3 mma.sync m16n8k32 u8 (bits expanded to bytes) */
+  int kappa;       /* multi-source width: 0 -> 64 | 32 | 64 | 128 (reading R19) */
+  int trace;       /* 0 | 1: keep the per-level trace (always cheap; default on) */
+  float eta;       /* bottom-up switch constant (Eq. 6, eta = 10 on Hopper); 0 -> library default */
+  float gamma;     /* slice-vs-edge-chunk byte ratio for the per-slice-set top-down choice; 0 -> default */
+  int reserved[6];
+} blest_options_t;
+
+typedef struct {
+  uint32_t n;
+  uint64_t nnz;
+  uint32_t n_slice_sets;   /* N_s = ceil(n / 8) */
+  uint32_t n_vss;          /* N_v = sum over slice sets of ceil(slices/128) */
+  uint64_t n_slices;       /* real (non-padding) slices */
+  uint64_t n_quads;        /* 4-slice groups stored (each slice set padded to a multiple of 4 slices) */
+  uint64_t bvss_bytes;     /* device bytes of rowIds + masks + setPtr */
+  uint64_t csr_bytes;      /* device bytes of rowptr + colidx */
+  uint64_t workspace_bytes;
+  double mask_density;     /* nnz / n_slices (rho_c, 1..8) */
+  double u_div;            /* update divergence (reading R20) */
+  double reorder_seconds, build_seconds, upload_seconds;
+  int kernel_chosen;       /* 1 eager | 2 lazy (after auto dispatch) */
+  int reorder, kappa, num_sms, grid_blocks, block_threads;
+  uint32_t queue_capacity; /* entries per work queue */
+} blest_info_t;
+
+/* One record per BFS level of the most recent blest_bfs call (written by the persistent kernel). */
+typedef struct {
+  uint32_t level;       /* l (1-based: vertices discovered in this record got level l) */
+  uint32_t mode;        /* 0 queue (slice chunks and/or edge chunks) | 1 bottom-up | 2 eager queue */
+  uint32_t q_entries;   /* work-queue entries consumed */
+  uint32_t new_vertices;
+  uint64_t q_bytes;     /* graph bytes the queue entries cover (20 B per quad, 4 B per edge) */
+  uint64_t bu_scanned;  /* bottom-up: neighbours scanned */
+  uint32_t unvisited;   /* after this level */
+  uint32_t reserved;
+  uint64_t t_ns;        /* %globaltimer at the end of the level, relative to kernel start */
+} blest_level_trace_t;
+
+/* Build: (optional reorder) -> BVSS -> U_div + dispatch -> upload.
+ * Synchronous.  opt == NULL => defaults.  Timed separately from traversal; see blest_get_info. */
+int blest_build(const blest_csr_t *csr, const blest_options_t *opt, blest_handle_t *out);
+
+/* Host-only pre-processing: the same reorder -> BVSS -> U_div pipeline as blest_build, without touching a device
+ * (csr->on_device must be 0).  The handle answers blest_get_info / blest_get_array only; traversal calls return
+ * BLEST_EUNSUPPORTED.  Used by the CPU tests of the host logic and for offline inspection. */
+int blest_preprocess_host(const blest_csr_t *csr, const blest_options_t *opt, blest_handle_t *out);
+
+/* Change the run-time options (kernel, switching, contraction, kappa, trace, eta, gamma). */
+int blest_configure(blest_handle_t h, const blest_options_t *opt);
+
+/* Single-source BFS (Alg. 2/3/4; one persistent cooperative kernel).
+ * levels_out: int32[n], device or host; levels_out[v] = hop distance from src, 0 for src, -1 if unreachable. */
+int blest_bfs(blest_handle_t h, uint32_t src, int32_t *levels_out, void *cuda_stream);
+
+/* Multi-source BFS (Alg. 5): srcs host uint32[k], k >= 1 (batched by kappa inside; duplicates legal).
+ * levels_out: int32[k*n], device or host; row b belongs to srcs[b], original ids, -1 = unreachable. */
+int blest_msbfs(blest_handle_t h, const uint32_t *srcs, uint32_t k, int32_t *levels_out, void *cuda_stream);
+
+/* Closeness centrality (Eq. 7-8; readings R13/R14): out[i] = (reach_i - 1) / far_i in fp64, 0.0 when
+ * far_i = 0.  srcs host uint32[n_srcs], or NULL = all vertices 0..n-1 (then n_srcs must be n; uses the paper's
+ * target-side accumulation).  out: double[n_srcs], device or host. */
+int blest_closeness(blest_handle_t h, const uint32_t *srcs, uint64_t n_srcs, double *out, void *cuda_stream);
+
+/* Same traversal as blest_closeness, returning the exact integers: far_out uint64[n_srcs] (sum of hop distances
+ * to all reachable vertices), reach_out uint32[n_srcs] (reachable vertices including the source).  Either may be NULL. */
+int blest_farness(blest_handle_t h, const uint32_t *srcs, uint64_t n_srcs, uint64_t *far_out, uint32_t *reach_out,
+                  void *cuda_stream);
+
+int blest_get_info(blest_handle_t h, blest_info_t *info);
+
+/* Per-level trace of the last blest_bfs call.  Synchronises the device.  *n_levels = records available
+ * (may exceed cap; only min(cap, available) are copied). */
+int blest_get_trace(blest_handle_t h, blest_level_trace_t *buf, uint32_t cap, uint32_t *n_levels);
+
+/* Copy one internal array to a HOST buffer (tests: BVSS round trip, permutation bijection).  `which`:
+ * 0 setPtr uint32[N_s+1] (quad offsets) | 1 rowIds uint32[4*n_quads] | 2 masks uint32[n_quads] |
+ * 3 realPtrs uint32[N_s+1] | 4 virtualToReal uint32[N_v] | 5 perm uint32[n] (orig -> internal) |
+ * 6 iperm uint32[n] | 7 internal rowptr uint32[n+1] | 8 internal colidx uint32[nnz].
+ * bytes must equal the array size exactly. */
+int blest_get_array(blest_handle_t h, int which, void *host_dst, uint64_t bytes);
+
+/* getVI(u, rho) = (u mod 8) * rho + floor(u / 8): the multi-source re-indexing, exported for tests. */
+uint64_t blest_get_vi(uint64_t u, uint64_t rho);
+
+/* Exhaustive device self-test of one contraction form against (mask & alpha) != 0 over all 2^8 x 2^8 pairs in
+ * all four byte positions.  *n_mismatch = differing results (0 = pass). */
+int blest_contraction_selftest(int contraction, uint64_t *n_mismatch);
+
+/* Tensor-pipe peak microbenchmark: issues `iters` dependent-free MMA instructions per warp on every SM and
+ * reports tera-ops/s (one op = one multiply-accumulate on one bit (b1) or one byte (u8)), 2 ops per MAC not applied.
+ * kind: 2 = mma.sync m8n8k128 b1 and.popc | 3 = mma.sync m16n8k32 u8. */
+int blest_mma_microbench(int kind, uint32_t iters, double *tera_macs_per_s, double *milliseconds);
+
+/* Grid-barrier latency microbenchmark: `iters` back-to-back grid barriers in the persistent launch configuration. */
+int blest_barrier_microbench(uint32_t iters, double *ns_per_barrier);
+
+void blest_destroy(blest_handle_t h);
+const char *blest_strerror(int status);
+int blest_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BLEST_H */

@@ -1,0 +1,10 @@
+"""blest-b200: B200-native (sm_100a) BLEST hot path -- BFS / multi-source BFS / closeness over a Binarized
+Virtual Slice Set, behind the C ABI of ``include/blest.h``.  See DESIGN.md.
+
+``binding`` is a thin ctypes layer (argument marshalling only); the product is ``libblest.so``.
+"""
+from .binding import (BlestError, Graph, Info, barrier_microbench, contraction_selftest, get_vi, load,  # noqa: F401
+                      mma_microbench, strerror)
+
+__all__ = ["BlestError", "Graph", "Info", "barrier_microbench", "contraction_selftest", "get_vi", "load",
+           "mma_microbench", "strerror"]

@@ -1,0 +1,602 @@
+// api.cu -- the C ABI of include/blest.h: handle lifetime, device memory, launches.  No traversal arithmetic here.
+#include <algorithm>
+#include <chrono>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "bfs_kernels.cuh"
+#include "host_graph.h"
+
+namespace blest {
+cudaError_t run_contraction_selftest(int contraction, unsigned long long* dMismatch);
+cudaError_t run_mma_peak(int kind, uint32_t iters, int blocks, int* dSink, double* macsPerLaunch);
+cudaError_t run_barrier_bench(unsigned int* dBar, uint32_t iters, int blocks, unsigned long long* dNs);
+}  // namespace blest
+
+using namespace blest;
+
+static thread_local int g_lastCuda = 0;
+
+#define CK(call)                                  \
+  do {                                            \
+    cudaError_t e__ = (call);                     \
+    if (e__ != cudaSuccess) {                     \
+      g_lastCuda = (int)e__;                      \
+      cudaGetLastError();                         \
+      return e__ == cudaErrorMemoryAllocation ? BLEST_ENOMEM : BLEST_ECUDA; \
+    }                                             \
+  } while (0)
+
+static constexpr uint32_t TRACE_CAP = 1u << 17;
+static constexpr double UDIV_THRESHOLD = 25000.0;
+
+struct blest_graph {
+  uint32_t n = 0, Ns = 0, Nv = 0, nwords = 0, rho = 0, qcap = 0;
+  uint64_t nnz = 0, nSlices = 0, nQuads = 0;
+  blest_options_t opt{};
+  blest_info_t info{};
+  bool hasPerm = false;
+  bool hostOnly = false;  // blest_preprocess_host: no device arrays, traversal calls are refused
+  HostBvss hb;            // kept only when hostOnly
+  HostCsr hcsr;           // kept only when hostOnly
+  std::vector<uint32_t> perm, iperm, realPtrs, virtualToReal;
+  int gridLazy = 0, gridEager = 0, gridMs = 0;
+  // device graph
+  uint32_t *dSetPtr = nullptr, *dRowIds = nullptr, *dMasks = nullptr, *dRowptr = nullptr, *dColidx = nullptr;
+  uint32_t *dPerm = nullptr, *dIperm = nullptr;
+  // single-source workspace
+  uint32_t *dVc = nullptr, *dVn = nullptr, *dF = nullptr;
+  uint2* dQ[2] = {nullptr, nullptr};
+  Ctrl* dCtrl = nullptr;
+  blest_level_trace_t* dTrace = nullptr;
+  int32_t *dL = nullptr, *dStamp = nullptr, *dOut = nullptr;
+  // multi-source workspace (allocated on first use for the current kappa)
+  int msKappa = 0;
+  uint32_t *dMsF = nullptr, *dMsVc = nullptr, *dMsVn = nullptr;
+  uint8_t* dDirty = nullptr;
+  unsigned long long* dFarT = nullptr;
+  uint32_t* dReachT = nullptr;
+  uint64_t wsBytes = 0;
+  std::vector<void*> allocs;
+};
+
+template <class T>
+static int dev_alloc(blest_graph* g, T** p, uint64_t count, bool zero = false) {
+  uint64_t bytes = std::max<uint64_t>(count * sizeof(T), 16);
+  bytes = (bytes + 15) & ~15ull;
+  CK(cudaMalloc((void**)p, bytes));
+  g->allocs.push_back((void*)*p);
+  g->wsBytes += bytes;
+  if (zero) CK(cudaMemset(*p, 0, bytes));
+  return BLEST_OK;
+}
+
+static bool is_device_ptr(const void* p) {
+  cudaPointerAttributes a;
+  cudaError_t e = cudaPointerGetAttributes(&a, p);
+  if (e != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+static double now_s() {
+  return std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count();
+}
+
+static void normalise_options(blest_options_t& o) {
+  if (o.kappa == 0) o.kappa = 64;
+  if (o.eta <= 0.f) o.eta = 10.f;
+  if (o.gamma <= 0.f) o.gamma = 1.0f;
+}
+
+static int check_options(const blest_options_t& o) {
+  if (o.reorder < 0 || o.reorder > 2 || o.builder < 0 || o.builder > 1) return BLEST_EINVAL;
+  if (o.kernel < 0 || o.kernel > 2 || o.switching < 0 || o.switching > 5) return BLEST_EINVAL;
+  if (o.contraction < 0 || o.contraction > 3) return BLEST_EINVAL;
+  if (o.kappa != 0 && o.kappa != 32 && o.kappa != 64 && o.kappa != 128) return BLEST_EINVAL;
+  return BLEST_OK;
+}
+
+extern "C" {
+
+const char* blest_strerror(int status) {
+  switch (status) {
+    case BLEST_OK: return "ok";
+    case BLEST_EINVAL: return "invalid argument";
+    case BLEST_ERANGE: return "size out of range";
+    case BLEST_EUNSORTED: return "CSR rows are not sorted";
+    case BLEST_ENOTSYM: return "CSR is not structurally symmetric or has out-of-range column ids";
+    case BLEST_ENOMEM: return "out of memory";
+    case BLEST_ECUDA: return "CUDA error";
+    case BLEST_EUNSUPPORTED: return "unsupported device or option";
+    case BLEST_EOVERFLOW: return "internal work queue overflow";
+    default: return "unknown status";
+  }
+}
+
+int blest_last_cuda_error(void) { return g_lastCuda; }
+
+uint64_t blest_get_vi(uint64_t u, uint64_t rho) { return (u % SIGMA) * rho + u / SIGMA; }
+
+void blest_destroy(blest_handle_t h) {
+  if (!h) return;
+  for (void* p : h->allocs) cudaFree(p);
+  delete h;
+}
+
+static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, blest_handle_t* out, bool hostOnly) {
+  if (!csr || !out || !csr->rowptr || (!csr->colidx && csr->nnz)) return BLEST_EINVAL;
+  *out = nullptr;
+  blest_options_t opt{};
+  if (optIn) opt = *optIn;
+  int rc = check_options(opt);
+  if (rc) return rc;
+  normalise_options(opt);
+  if (csr->n == 0 || csr->n > (1u << 29) || csr->nnz > 0xFFFFFFFFull) return BLEST_ERANGE;
+  if (opt.builder == 1) return BLEST_EUNSUPPORTED;  // device builder: not in this round
+  if (hostOnly && csr->on_device) return BLEST_EINVAL;
+
+  int sms = 0;
+  if (!hostOnly) {
+    int dev = 0, major = 0, coop = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (major != 10 || !coop) return BLEST_EUNSUPPORTED;
+  }
+
+  blest_graph* g = new (std::nothrow) blest_graph();
+  if (!g) return BLEST_ENOMEM;
+  g->hostOnly = hostOnly;
+  struct Guard { blest_graph* g; ~Guard() { if (g) blest_destroy(g); } } guard{g};
+
+  try {
+    HostCsr in;
+    in.n = csr->n;
+    in.nnz = csr->nnz;
+    in.rowptr.resize((size_t)csr->n + 1);
+    in.colidx.resize((size_t)csr->nnz);
+    if (csr->on_device) {
+      CK(cudaMemcpy(in.rowptr.data(), csr->rowptr, in.rowptr.size() * 4, cudaMemcpyDeviceToHost));
+      if (csr->nnz) CK(cudaMemcpy(in.colidx.data(), csr->colidx, in.colidx.size() * 4, cudaMemcpyDeviceToHost));
+    } else {
+      std::memcpy(in.rowptr.data(), csr->rowptr, in.rowptr.size() * 4);
+      if (csr->nnz) std::memcpy(in.colidx.data(), csr->colidx, in.colidx.size() * 4);
+    }
+    rc = check_csr(in, opt.validate != 0);
+    if (rc) return rc;
+
+    // A1 reorder (timed separately, Table 7)
+    double t0 = now_s();
+    HostCsr work;
+    HostCsr* gcsr = &in;
+    if (opt.reorder) {
+      make_permutation(in, opt.reorder, g->perm);
+      g->iperm.resize(in.n);
+      for (uint32_t i = 0; i < in.n; ++i) g->iperm[g->perm[i]] = i;
+      relabel_csr(in, g->perm, work);
+      std::vector<uint32_t>().swap(in.colidx);
+      std::vector<uint32_t>().swap(in.rowptr);
+      gcsr = &work;
+      g->hasPerm = true;
+    }
+    g->info.reorder_seconds = now_s() - t0;
+
+    // A2 BVSS build + A3 statistics
+    t0 = now_s();
+    HostBvss b;
+    rc = build_bvss(*gcsr, b);
+    if (rc) return rc;
+    g->info.build_seconds = now_s() - t0;
+
+    g->n = gcsr->n;
+    g->nnz = gcsr->nnz;
+    g->Ns = b.Ns;
+    g->Nv = b.Nv;
+    g->rho = b.Ns;  // rho = ceil(n / sigma)
+    g->nSlices = b.nSlices;
+    g->nQuads = b.nQuads;
+    g->nwords = (g->n + 31) / 32;
+    g->realPtrs.swap(b.realPtrs);
+    g->virtualToReal.swap(b.virtualToReal);
+    g->opt = opt;
+    const double uDiv = b.uDiv;
+
+    if (hostOnly) {
+      g->info.bvss_bytes = ((uint64_t)g->Ns + 1) * 4 + g->nQuads * 20;
+      g->info.csr_bytes = ((uint64_t)g->n + 1) * 4 + g->nnz * 4;
+      g->hb = std::move(b);
+      g->hcsr = std::move(*gcsr);
+    } else {
+      // upload
+      t0 = now_s();
+      uint64_t before = g->wsBytes;
+      if ((rc = dev_alloc(g, &g->dSetPtr, (uint64_t)g->Ns + 1))) return rc;
+      if ((rc = dev_alloc(g, &g->dRowIds, g->nQuads * 4))) return rc;
+      if ((rc = dev_alloc(g, &g->dMasks, g->nQuads))) return rc;
+      g->info.bvss_bytes = g->wsBytes - before;
+      before = g->wsBytes;
+      if ((rc = dev_alloc(g, &g->dRowptr, (uint64_t)g->n + 1))) return rc;
+      if ((rc = dev_alloc(g, &g->dColidx, g->nnz))) return rc;
+      g->info.csr_bytes = g->wsBytes - before;
+      CK(cudaMemcpy(g->dSetPtr, b.setPtr.data(), ((size_t)g->Ns + 1) * 4, cudaMemcpyHostToDevice));
+      if (g->nQuads) {
+        CK(cudaMemcpy(g->dRowIds, b.rowIds.data(), (size_t)g->nQuads * 16, cudaMemcpyHostToDevice));
+        CK(cudaMemcpy(g->dMasks, b.masks.data(), (size_t)g->nQuads * 4, cudaMemcpyHostToDevice));
+      }
+      CK(cudaMemcpy(g->dRowptr, gcsr->rowptr.data(), ((size_t)g->n + 1) * 4, cudaMemcpyHostToDevice));
+      if (g->nnz) CK(cudaMemcpy(g->dColidx, gcsr->colidx.data(), (size_t)g->nnz * 4, cudaMemcpyHostToDevice));
+      if (g->hasPerm) {
+        if ((rc = dev_alloc(g, &g->dPerm, g->n))) return rc;
+        if ((rc = dev_alloc(g, &g->dIperm, g->n))) return rc;
+        CK(cudaMemcpy(g->dPerm, g->perm.data(), (size_t)g->n * 4, cudaMemcpyHostToDevice));
+        CK(cudaMemcpy(g->dIperm, g->iperm.data(), (size_t)g->n * 4, cudaMemcpyHostToDevice));
+      }
+      g->info.upload_seconds = now_s() - t0;
+      { HostBvss drop; std::swap(drop, b); }  // release the host copy
+
+      // workspace
+      const uint64_t qcap64 = (uint64_t)g->Nv + g->n + g->nnz / TD_CHUNK + 1024;
+      if (qcap64 > 0xFFFFFFF0ull) return BLEST_ERANGE;
+      g->qcap = (uint32_t)qcap64;
+      if ((rc = dev_alloc(g, &g->dVc, (uint64_t)g->nwords + 4, true))) return rc;
+      if ((rc = dev_alloc(g, &g->dVn, (uint64_t)g->nwords + 4, true))) return rc;
+      if ((rc = dev_alloc(g, &g->dF, (uint64_t)g->nwords + 4, true))) return rc;
+      if ((rc = dev_alloc(g, &g->dQ[0], g->qcap))) return rc;
+      if ((rc = dev_alloc(g, &g->dQ[1], g->qcap))) return rc;
+      if ((rc = dev_alloc(g, &g->dCtrl, 1, true))) return rc;
+      if ((rc = dev_alloc(g, &g->dTrace, TRACE_CAP, true))) return rc;
+      if ((rc = dev_alloc(g, &g->dStamp, g->Ns))) return rc;
+      if ((rc = dev_alloc(g, &g->dOut, g->n))) return rc;
+      if (g->hasPerm && (rc = dev_alloc(g, &g->dL, g->n))) return rc;
+
+      g->gridLazy = max_coop_blocks_lazy();
+      g->gridEager = max_coop_blocks_eager();
+      g->gridMs = max_coop_blocks_msbfs();
+      if (g->gridLazy <= 0 || g->gridEager <= 0 || g->gridMs <= 0) return BLEST_EUNSUPPORTED;
+    }
+
+    blest_info_t& I = g->info;
+    I.n = g->n;
+    I.nnz = g->nnz;
+    I.n_slice_sets = g->Ns;
+    I.n_vss = g->Nv;
+    I.n_slices = g->nSlices;
+    I.n_quads = g->nQuads;
+    I.mask_density = g->nSlices ? (double)g->nnz / (double)g->nSlices : 0.0;
+    I.u_div = uDiv;
+    I.reorder = opt.reorder;
+    I.num_sms = sms;
+    I.grid_blocks = g->gridLazy;
+    I.block_threads = BLOCK_THREADS;
+    I.queue_capacity = g->qcap;
+  } catch (const std::bad_alloc&) {
+    return BLEST_ENOMEM;
+  }
+  guard.g = nullptr;
+  *out = g;
+  return BLEST_OK;
+}
+
+int blest_build(const blest_csr_t* csr, const blest_options_t* opt, blest_handle_t* out) {
+  return build_impl(csr, opt, out, false);
+}
+
+int blest_preprocess_host(const blest_csr_t* csr, const blest_options_t* opt, blest_handle_t* out) {
+  return build_impl(csr, opt, out, true);
+}
+
+int blest_configure(blest_handle_t h, const blest_options_t* optIn) {
+  if (!h || !optIn) return BLEST_EINVAL;
+  blest_options_t o = *optIn;
+  o.reorder = h->opt.reorder;
+  o.builder = h->opt.builder;
+  o.validate = h->opt.validate;
+  int rc = check_options(o);
+  if (rc) return rc;
+  normalise_options(o);
+  h->opt = o;
+  return BLEST_OK;
+}
+
+static int resolved_kernel(const blest_graph* g) {
+  if (g->opt.kernel) return g->opt.kernel;
+  return g->info.u_div > UDIV_THRESHOLD ? 2 : 1;
+}
+
+int blest_get_info(blest_handle_t h, blest_info_t* info) {
+  if (!h || !info) return BLEST_EINVAL;
+  h->info.kernel_chosen = resolved_kernel(h);
+  h->info.kappa = h->opt.kappa;
+  h->info.workspace_bytes = h->hostOnly ? 0 : h->wsBytes - h->info.bvss_bytes - h->info.csr_bytes;
+  *info = h->info;
+  return BLEST_OK;
+}
+
+int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_stream) {
+  if (!h || !levels_out) return BLEST_EINVAL;
+  if (h->hostOnly) return BLEST_EUNSUPPORTED;
+  if (src >= h->n) return BLEST_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const bool devOut = is_device_ptr(levels_out);
+  BfsParams p{};
+  p.n = h->n; p.Ns = h->Ns; p.nwords = h->nwords; p.qcap = h->qcap; p.nnz = h->nnz;
+  p.setPtr = h->dSetPtr; p.rowIds = reinterpret_cast<const uint4*>(h->dRowIds); p.masks = h->dMasks;
+  p.rowptr = h->dRowptr; p.colidx = h->dColidx; p.iperm = h->hasPerm ? h->dIperm : nullptr;
+  p.Vcurr = h->dVc; p.Vnext = h->dVn; p.Fcurr = h->dF;
+  p.Q[0] = h->dQ[0]; p.Q[1] = h->dQ[1];
+  p.out = devOut ? levels_out : h->dOut;
+  p.L = h->hasPerm ? h->dL : p.out;
+  p.stamp = h->dStamp;
+  p.ctrl = h->dCtrl;
+  p.trace = h->opt.trace == 0 || h->opt.trace == 1 ? h->dTrace : nullptr;
+  p.traceCap = TRACE_CAP;
+  p.src = h->hasPerm ? h->perm[src] : src;
+  p.switching = h->opt.switching;
+  p.contraction = h->opt.contraction ? h->opt.contraction : 1;  // auto -> ALU (measured fastest)
+  p.buMask = (uint32_t)h->opt.reserved[0];
+  p.eta = h->opt.eta;
+  p.gamma = h->opt.gamma;
+  CK(cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st));
+  if (resolved_kernel(h) == 1) CK(launch_bfs_eager(p, h->gridEager, st));
+  else CK(launch_bfs_lazy(p, h->gridLazy, st));
+  if (!devOut) CK(cudaMemcpyAsync(levels_out, h->dOut, (size_t)h->n * 4, cudaMemcpyDeviceToHost, st));
+  return BLEST_OK;
+}
+
+int blest_get_trace(blest_handle_t h, blest_level_trace_t* buf, uint32_t cap, uint32_t* n_levels) {
+  if (!h || !n_levels) return BLEST_EINVAL;
+  if (h->hostOnly) return BLEST_EUNSUPPORTED;
+  CK(cudaDeviceSynchronize());
+  Ctrl c;
+  CK(cudaMemcpy(&c, h->dCtrl, sizeof(Ctrl), cudaMemcpyDeviceToHost));
+  *n_levels = c.nlevels;
+  const uint32_t k = std::min(std::min(cap, c.nlevels), TRACE_CAP);
+  if (buf && k) CK(cudaMemcpy(buf, h->dTrace, (size_t)k * sizeof(blest_level_trace_t), cudaMemcpyDeviceToHost));
+  return (c.error & 1u) ? BLEST_EOVERFLOW : BLEST_OK;
+}
+
+static int ensure_ms_workspace(blest_graph* g) {
+  const int kappa = g->opt.kappa;
+  if (g->msKappa == kappa) return BLEST_OK;
+  int rc;
+  const uint64_t words = (uint64_t)g->rho * 8u * (kappa / 32) + 4;
+  // (re)allocation for a different kappa simply adds buffers; the old ones are freed with the handle
+  if ((rc = dev_alloc(g, &g->dMsF, words, true))) return rc;
+  if ((rc = dev_alloc(g, &g->dMsVc, words, true))) return rc;
+  if ((rc = dev_alloc(g, &g->dMsVn, words, true))) return rc;
+  if (!g->dDirty && (rc = dev_alloc(g, &g->dDirty, (uint64_t)g->Ns + 16, true))) return rc;
+  if (!g->dFarT && (rc = dev_alloc(g, &g->dFarT, (uint64_t)g->rho * 8u, true))) return rc;
+  if (!g->dReachT && (rc = dev_alloc(g, &g->dReachT, (uint64_t)g->rho * 8u, true))) return rc;
+  g->msKappa = kappa;
+  return BLEST_OK;
+}
+
+static void fill_ms_params(blest_graph* h, MsParams& p) {
+  p.n = h->n; p.Ns = h->Ns; p.rho = h->rho; p.qcap = h->qcap;
+  p.setPtr = h->dSetPtr; p.rowIds = reinterpret_cast<const uint4*>(h->dRowIds); p.masks = h->dMasks;
+  p.perm = h->hasPerm ? h->dPerm : nullptr;
+  p.iperm = h->hasPerm ? h->dIperm : nullptr;
+  p.F = h->dMsF; p.Vc = h->dMsVc; p.Vn = h->dMsVn; p.dirty = h->dDirty;
+  p.Q[0] = h->dQ[0]; p.Q[1] = h->dQ[1];
+  p.ctrl = h->dCtrl;
+  p.kappa = h->opt.kappa;
+}
+
+int blest_msbfs(blest_handle_t h, const uint32_t* srcs, uint32_t k, int32_t* levels_out, void* cuda_stream) {
+  if (!h || !srcs || !levels_out || k == 0) return BLEST_EINVAL;
+  if (h->hostOnly) return BLEST_EUNSUPPORTED;
+  for (uint32_t i = 0; i < k; ++i)
+    if (srcs[i] >= h->n) return BLEST_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = ensure_ms_workspace(h);
+  if (rc) return rc;
+  const bool devOut = is_device_ptr(levels_out);
+  uint32_t* dSrcs = nullptr;
+  int32_t* dLevels = nullptr;
+  CK(cudaMalloc((void**)&dSrcs, (size_t)k * 4));
+  if (!devOut) {
+    cudaError_t e = cudaMalloc((void**)&dLevels, (size_t)k * h->n * 4);
+    if (e != cudaSuccess) { cudaFree(dSrcs); g_lastCuda = (int)e; cudaGetLastError(); return BLEST_ENOMEM; }
+  }
+  auto cleanup = [&]() { cudaFree(dSrcs); if (dLevels) cudaFree(dLevels); };
+  cudaError_t e = cudaMemcpyAsync(dSrcs, srcs, (size_t)k * 4, cudaMemcpyHostToDevice, st);
+  MsParams p{};
+  fill_ms_params(h, p);
+  p.srcs = dSrcs;
+  p.nsrcs = k;
+  p.levels = devOut ? levels_out : dLevels;
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st);
+  if (e == cudaSuccess) e = launch_msbfs(p, h->gridMs, st);
+  if (e == cudaSuccess && !devOut)
+    e = cudaMemcpyAsync(levels_out, dLevels, (size_t)k * h->n * 4, cudaMemcpyDeviceToHost, st);
+  // the temporaries (and the host srcs array) must outlive the enqueued work: this call synchronises the stream
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cleanup();
+  if (e != cudaSuccess) { g_lastCuda = (int)e; cudaGetLastError(); return BLEST_ECUDA; }
+  return BLEST_OK;
+}
+
+static int closeness_impl(blest_handle_t h, const uint32_t* srcs, uint64_t n_srcs, double* cc, uint64_t* farOut,
+                          uint32_t* reachOut, void* cuda_stream) {
+  if (!h || n_srcs == 0) return BLEST_EINVAL;
+  if (h->hostOnly) return BLEST_EUNSUPPORTED;
+  if (!cc && !farOut && !reachOut) return BLEST_EINVAL;
+  if (!srcs && n_srcs != h->n) return BLEST_EINVAL;
+  if (srcs)
+    for (uint64_t i = 0; i < n_srcs; ++i)
+      if (srcs[i] >= h->n) return BLEST_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = ensure_ms_workspace(h);
+  if (rc) return rc;
+  uint32_t* dSrcs = nullptr;
+  unsigned long long *dFarS = nullptr, *dFarO = nullptr;
+  uint32_t *dReachS = nullptr, *dReachO = nullptr;
+  double* dCc = nullptr;
+  std::vector<void*> tmp;
+  auto talloc = [&](void** p, size_t bytes) -> cudaError_t {
+    cudaError_t e = cudaMalloc(p, std::max<size_t>(bytes, 16));
+    if (e == cudaSuccess) tmp.push_back(*p);
+    return e;
+  };
+  auto cleanup = [&]() { for (void* p : tmp) cudaFree(p); };
+  cudaError_t e = cudaSuccess;
+  const bool ccDev = cc && is_device_ptr(cc), farDev = farOut && is_device_ptr(farOut), reachDev = reachOut && is_device_ptr(reachOut);
+  MsParams p{};
+  fill_ms_params(h, p);
+  p.nsrcs = n_srcs;
+  if (srcs) {  // arbitrary subset: per-source counts (reading R13)
+    e = talloc((void**)&dSrcs, n_srcs * 4);
+    if (e == cudaSuccess) e = talloc((void**)&dFarS, n_srcs * 8);
+    if (e == cudaSuccess) e = talloc((void**)&dReachS, n_srcs * 4);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dSrcs, srcs, n_srcs * 4, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(dFarS, 0, n_srcs * 8, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(dReachS, 0, n_srcs * 4, st);
+    p.srcs = dSrcs;
+    p.farS = dFarS;
+    p.reachS = dReachS;
+  } else {  // all vertices: the paper's target-side accumulation (Eq. 7)
+    e = cudaMemsetAsync(h->dFarT, 0, (size_t)h->rho * 8u * 8u, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->dReachT, 0, (size_t)h->rho * 8u * 4u, st);
+    p.farT = h->dFarT;
+    p.reachT = h->dReachT;
+  }
+  if (e == cudaSuccess && cc && !ccDev) e = talloc((void**)&dCc, n_srcs * 8);
+  if (e == cudaSuccess && farOut && !farDev) e = talloc((void**)&dFarO, n_srcs * 8);
+  if (e == cudaSuccess && reachOut && !reachDev) e = talloc((void**)&dReachO, n_srcs * 4);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st);
+  if (e == cudaSuccess) e = launch_msbfs(p, h->gridMs, st);
+  if (e == cudaSuccess)
+    e = launch_closeness_finalize(h->n, h->rho, h->hasPerm ? h->dPerm : nullptr, p.farT, p.reachT, p.farS, p.reachS, n_srcs,
+                                  cc ? (ccDev ? cc : dCc) : nullptr,
+                                  farOut ? (farDev ? (unsigned long long*)farOut : dFarO) : nullptr,
+                                  reachOut ? (reachDev ? reachOut : dReachO) : nullptr, st);
+  if (e == cudaSuccess && cc && !ccDev) e = cudaMemcpyAsync(cc, dCc, n_srcs * 8, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && farOut && !farDev) e = cudaMemcpyAsync(farOut, dFarO, n_srcs * 8, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && reachOut && !reachDev) e = cudaMemcpyAsync(reachOut, dReachO, n_srcs * 4, cudaMemcpyDeviceToHost, st);
+  const bool needSync = !tmp.empty();
+  if (e == cudaSuccess && needSync) e = cudaStreamSynchronize(st);
+  cleanup();
+  if (e != cudaSuccess) {
+    g_lastCuda = (int)e;
+    cudaGetLastError();
+    return e == cudaErrorMemoryAllocation ? BLEST_ENOMEM : BLEST_ECUDA;
+  }
+  return BLEST_OK;
+}
+
+int blest_closeness(blest_handle_t h, const uint32_t* srcs, uint64_t n_srcs, double* out, void* cuda_stream) {
+  if (!out) return BLEST_EINVAL;
+  return closeness_impl(h, srcs, n_srcs, out, nullptr, nullptr, cuda_stream);
+}
+
+int blest_farness(blest_handle_t h, const uint32_t* srcs, uint64_t n_srcs, uint64_t* far_out, uint32_t* reach_out,
+                  void* cuda_stream) {
+  return closeness_impl(h, srcs, n_srcs, nullptr, far_out, reach_out, cuda_stream);
+}
+
+int blest_get_array(blest_handle_t h, int which, void* host_dst, uint64_t bytes) {
+  if (!h || !host_dst) return BLEST_EINVAL;
+  const void* src = nullptr;
+  uint64_t want = 0;
+  bool onHost = false;
+  switch (which) {
+    case 0: src = h->dSetPtr; want = ((uint64_t)h->Ns + 1) * 4; break;
+    case 1: src = h->dRowIds; want = h->nQuads * 16; break;
+    case 2: src = h->dMasks; want = h->nQuads * 4; break;
+    case 3: src = h->realPtrs.data(); want = ((uint64_t)h->Ns + 1) * 4; onHost = true; break;
+    case 4: src = h->virtualToReal.data(); want = (uint64_t)h->Nv * 4; onHost = true; break;
+    case 5: if (!h->hasPerm) return BLEST_EINVAL; src = h->perm.data(); want = (uint64_t)h->n * 4; onHost = true; break;
+    case 6: if (!h->hasPerm) return BLEST_EINVAL; src = h->iperm.data(); want = (uint64_t)h->n * 4; onHost = true; break;
+    case 7: src = h->dRowptr; want = ((uint64_t)h->n + 1) * 4; break;
+    case 8: src = h->dColidx; want = h->nnz * 4; break;
+    default: return BLEST_EINVAL;
+  }
+  if (h->hostOnly) {
+    onHost = true;
+    switch (which) {
+      case 0: src = h->hb.setPtr.data(); break;
+      case 1: src = h->hb.rowIds.data(); break;
+      case 2: src = h->hb.masks.data(); break;
+      case 7: src = h->hcsr.rowptr.data(); break;
+      case 8: src = h->hcsr.colidx.data(); break;
+      default: break;
+    }
+  }
+  if (bytes != want) return BLEST_EINVAL;
+  if (want == 0) return BLEST_OK;
+  if (onHost) std::memcpy(host_dst, src, want);
+  else CK(cudaMemcpy(host_dst, src, want, cudaMemcpyDeviceToHost));
+  return BLEST_OK;
+}
+
+int blest_contraction_selftest(int contraction, uint64_t* n_mismatch) {
+  if (!n_mismatch || contraction < 1 || contraction > 3) return BLEST_EINVAL;
+  unsigned long long* d = nullptr;
+  CK(cudaMalloc((void**)&d, 8));
+  cudaError_t e = cudaMemset(d, 0, 8);
+  if (e == cudaSuccess) e = run_contraction_selftest(contraction, d);
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  unsigned long long v = 0;
+  if (e == cudaSuccess) e = cudaMemcpy(&v, d, 8, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  CK(e);
+  *n_mismatch = v;
+  return BLEST_OK;
+}
+
+int blest_mma_microbench(int kind, uint32_t iters, double* tera_macs_per_s, double* milliseconds) {
+  if (!tera_macs_per_s || (kind != 2 && kind != 3) || iters == 0) return BLEST_EINVAL;
+  int dev = 0, sms = 0;
+  CK(cudaGetDevice(&dev));
+  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  int* dSink = nullptr;
+  CK(cudaMalloc((void**)&dSink, 4));
+  cudaEvent_t a, b;
+  cudaEventCreate(&a);
+  cudaEventCreate(&b);
+  double macs = 0;
+  cudaError_t e = run_mma_peak(kind, iters, sms, dSink, &macs);  // warm-up
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  float best = 1e30f;
+  for (int rep = 0; rep < 5 && e == cudaSuccess; ++rep) {
+    cudaEventRecord(a);
+    e = run_mma_peak(kind, iters, sms, dSink, &macs);
+    cudaEventRecord(b);
+    if (e == cudaSuccess) e = cudaEventSynchronize(b);
+    float ms = 0;
+    cudaEventElapsedTime(&ms, a, b);
+    best = std::min(best, ms);
+  }
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  cudaFree(dSink);
+  CK(e);
+  *tera_macs_per_s = macs / (best * 1e-3) / 1e12;
+  if (milliseconds) *milliseconds = best;
+  return BLEST_OK;
+}
+
+int blest_barrier_microbench(uint32_t iters, double* ns_per_barrier) {
+  if (!ns_per_barrier || iters == 0) return BLEST_EINVAL;
+  int dev = 0, sms = 0;
+  CK(cudaGetDevice(&dev));
+  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  unsigned int* dBar = nullptr;
+  unsigned long long* dNs = nullptr;
+  CK(cudaMalloc((void**)&dBar, 16));
+  cudaError_t e = cudaMalloc((void**)&dNs, 8);
+  if (e == cudaSuccess) e = cudaMemset(dBar, 0, 16);
+  if (e == cudaSuccess) e = run_barrier_bench(dBar, iters, sms, dNs);
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  unsigned long long ns = 0;
+  if (e == cudaSuccess) e = cudaMemcpy(&ns, dNs, 8, cudaMemcpyDeviceToHost);
+  cudaFree(dBar);
+  if (dNs) cudaFree(dNs);
+  CK(e);
+  *ns_per_barrier = (double)ns / iters;
+  return BLEST_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,268 @@
+// msbfs_kernels.cu -- bit-packed multi-source BFS (§6.1, Alg. 5) and closeness accumulation (§6.2, Eq. 7-8).
+//
+// kappa = 32*KW BFS instances share one kappa-bit word per vertex, stored at getVI(u, rho) = (u mod 8)*rho + u/8
+// so that Stage 2's thread-per-slice-set sweep is coalesced.  One persistent cooperative kernel
+// loops over ALL source batches (PAPER.md:635 invokes the kernel ceil(n/kappa) times; here the batch loop is
+// inside the kernel, so a closeness run is a single launch).
+//
+// Contraction: Alg. 5 lines 16-30 loop over the active BFS instances c with one ballot + two MMAs each.  On sm_100a
+// there is no binary MMA; the same Boolean product [128 slices x 8] x [8 x kappa] is evaluated for all kappa
+// instances at once as M = OR_{j in mask} F_curr^kappa[column j]  (8 selected ORs of kappa-bit words per slice).
+// The per-instance loop, and with it activeSets, disappears; the per-set OR "A" of Alg. 5 line 51
+// still decides which slice sets are enqueued.  dirtySets is kept as in the paper.
+#include "bfs_kernels.cuh"
+
+namespace blest {
+
+namespace {
+
+struct MsShared {
+  BigSeg bigList[WARPS_PER_BLOCK][BIG_CAP];
+  uint32_t bigCnt[WARPS_PER_BLOCK];
+  unsigned long long acc;
+  uint32_t perSource[128];
+};
+
+template <int KW>
+__device__ __forceinline__ void ms_stage1(const MsParams& p, const uint2* Qc, uint32_t qcount) {
+  const uint32_t lane = threadIdx.x & 31;
+  const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
+  for (uint32_t i = gwarp; i < qcount; i += nwarps) {
+    const uint2 e = Qc[i];
+    const uint32_t nq = (e.y & 31u) + 1u, s = e.y >> 5;
+    uint4 rows = make_uint4(0, 0, 0, 0);
+    uint32_t m = 0;
+    if (lane < nq) {
+      rows = __ldg(p.rowIds + e.x + lane);
+      m = __ldg(p.masks + e.x + lane);
+    }
+    // the first sigma lanes gather the kappa-bit frontier words of the set's 8 columns
+    uint32_t fv[KW];
+#pragma unroll
+    for (int w = 0; w < KW; ++w) fv[w] = 0;
+    if (lane < 8) {
+      const uint64_t idx = (uint64_t)lane * p.rho + s;
+#pragma unroll
+      for (int w = 0; w < KW; ++w) fv[w] = p.F[idx * KW + w];
+    }
+    uint32_t f[8][KW];
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+#pragma unroll
+      for (int w = 0; w < KW; ++w) f[j][w] = __shfl_sync(0xffffffffu, fv[w], j);
+    const uint32_t ru[4] = {rows.x, rows.y, rows.z, rows.w};
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      const uint32_t mb = (m >> (8 * c)) & 0xFFu;
+      if (mb) {
+        uint32_t M[KW];  // per-row kappa-bit accumulation buffer ("M[0..3]")
+#pragma unroll
+        for (int w = 0; w < KW; ++w) M[w] = 0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const uint32_t sel = 0u - ((mb >> j) & 1u);
+#pragma unroll
+          for (int w = 0; w < KW; ++w) M[w] |= f[j][w] & sel;
+        }
+        const uint32_t u = ru[c];
+        const uint64_t idx = (uint64_t)(u & 7u) * p.rho + (u >> 3);  // getVI(u, rho)
+        bool any = false;
+#pragma unroll
+        for (int w = 0; w < KW; ++w) {
+          if (M[w]) {
+            const uint32_t fresh = M[w] & ~__ldcg(&p.Vn[idx * KW + w]);
+            if (fresh) { atomicOr(&p.Vn[idx * KW + w], fresh); any = true; }  // one RED per row
+          }
+        }
+        if (any) p.dirty[u >> 3] = 1;  // PAPER.md:583 dirtySets
+      }
+    }
+  }
+}
+
+template <int KW>
+__device__ __forceinline__ void ms_stage2(const MsParams& p, MsShared& sh, uint32_t level, uint64_t b0, uint32_t nb,
+                                          uint2* Qn, unsigned int* qcn, uint32_t par) {
+  const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + warp, nwarps = gridDim.x * WARPS_PER_BLOCK;
+  BigSeg* bigList = sh.bigList[warp];
+  uint32_t* bigCnt = &sh.bigCnt[warp];
+  unsigned long long nnew = 0;
+  const bool perSource = (p.farS != nullptr) || (p.reachS != nullptr);
+  for (uint64_t sb = (uint64_t)gwarp * 32; sb < p.Ns; sb += (uint64_t)nwarps * 32) {
+    const uint32_t s = (uint32_t)sb + lane;  // consecutive threads -> consecutive slice sets
+    uint32_t cnt = 0, a = 0, nq = 0;
+    if (s < p.Ns && p.dirty[s]) {  // skip slice sets nobody marked
+      p.dirty[s] = 0;
+      uint32_t A = 0;
+#pragma unroll
+      for (uint32_t j = 0; j < 8; ++j) {
+        const uint64_t idx = (uint64_t)j * p.rho + s;
+        uint32_t pc = 0;
+#pragma unroll
+        for (int w = 0; w < KW; ++w) {
+          const uint32_t next = p.Vn[idx * KW + w], cur = p.Vc[idx * KW + w];
+          const uint32_t diff = next ^ cur;
+          p.F[idx * KW + w] = diff;  // PAPER.md:610 (unconditional)
+          if (diff) {
+            p.Vc[idx * KW + w] = next;
+            A |= diff;
+            pc += __popc(diff);
+            if (perSource || p.levels) {
+              const uint32_t u = s * 8u + j;
+              const uint32_t uo = p.iperm ? __ldg(&p.iperm[u]) : u;
+              for (uint32_t d = diff; d; d &= d - 1) {
+                const uint32_t c = w * 32u + (__ffs(d) - 1);
+                if (perSource) atomicAdd(&sh.perSource[c], 1u);
+                if (p.levels) p.levels[(b0 + c) * (uint64_t)p.n + uo] = (int32_t)level;
+              }
+            }
+          }
+        }
+        if (pc) {
+          nnew += pc;
+          if (p.farT) p.farT[idx] += (unsigned long long)level * pc;  // Eq. 7: far[idx] += l * popc(diff)
+          if (p.reachT) p.reachT[idx] += pc;
+        }
+      }
+      if (A) {  // active in at least one BFS: enqueue all VSSs of the set
+        a = __ldg(&p.setPtr[s]);
+        nq = __ldg(&p.setPtr[s + 1]) - a;
+        cnt = seg_entries(0, nq);
+      }
+    }
+    bool ok;
+    uint32_t pos = warp_reserve(qcn, cnt, lane, p.qcap, &p.ctrl->error, ok);
+    if (cnt && ok) emit_segment(Qn, pos, 0, a, nq, s, bigList, bigCnt);
+    flush_big_segments(Qn, bigList, bigCnt, lane);
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) nnew += __shfl_down_sync(0xffffffffu, nnew, d);
+  if (lane == 0 && nnew) atomicAdd(&sh.acc, nnew);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    if (sh.acc) atomicAdd(&p.ctrl->newcount[par], sh.acc);
+    sh.acc = 0;
+  }
+  if (perSource && threadIdx.x < nb) {
+    const uint32_t k = sh.perSource[threadIdx.x];
+    if (k) {
+      if (p.farS) atomicAdd(&p.farS[b0 + threadIdx.x], (unsigned long long)level * k);
+      if (p.reachS) atomicAdd(&p.reachS[b0 + threadIdx.x], k);
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < 128) sh.perSource[threadIdx.x] = 0;
+  __syncthreads();
+}
+
+template <int KW>
+__global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_constant__ MsParams p) {
+  __shared__ MsShared sh;
+  constexpr uint32_t KAPPA = 32u * KW;
+  unsigned int epoch = 0;
+  Ctrl* ctrl = p.ctrl;
+  const uint64_t gtid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (uint64_t)gridDim.x * blockDim.x;
+  if (threadIdx.x < WARPS_PER_BLOCK) sh.bigCnt[threadIdx.x] = 0;
+  if (threadIdx.x < 128) sh.perSource[threadIdx.x] = 0;
+  if (threadIdx.x == 0) sh.acc = 0;
+  __syncthreads();
+  const uint64_t stateWords = (uint64_t)p.rho * 8u * KW;
+
+  for (uint64_t b0 = 0; b0 < p.nsrcs; b0 += KAPPA) {
+    const uint32_t nb = (uint32_t)min((uint64_t)KAPPA, p.nsrcs - b0);
+    // init(srcs, ...) (reading R16): visited words cleared, bit c of source c set, its set marked dirty
+    grid_fill32(p.Vc, 0u, stateWords);
+    grid_fill32(p.Vn, 0u, stateWords);
+    if (p.levels) {
+      uint32_t* base = reinterpret_cast<uint32_t*>(p.levels + b0 * (uint64_t)p.n);
+      for (uint64_t i = gtid; i < (uint64_t)nb * p.n; i += nth) base[i] = 0xFFFFFFFFu;
+    }
+    grid_barrier(&ctrl->bar, epoch);
+    if (gtid < nb) {
+      const uint32_t c = (uint32_t)gtid;
+      const uint32_t so = p.srcs ? p.srcs[b0 + c] : (uint32_t)(b0 + c);
+      const uint32_t si = p.perm ? __ldg(&p.perm[so]) : so;
+      const uint64_t idx = (uint64_t)(si & 7u) * p.rho + (si >> 3);
+      atomicOr(&p.Vn[idx * KW + (c >> 5)], 1u << (c & 31u));
+      p.dirty[si >> 3] = 1;
+    }
+    grid_barrier(&ctrl->bar, epoch);
+    // level 0 = the finalisation sweep over the sources themselves (far += 0, reach += 1, level 0, enqueue their sets)
+    ms_stage2<KW>(p, sh, 0, b0, nb, p.Q[1], &ctrl->qc[1], 0);
+    grid_barrier(&ctrl->bar, epoch);
+    for (uint32_t level = 1;; ++level) {
+      const uint32_t pp = (level - 1) & 1u, par = level & 1u;
+      if (ld_volatile(&ctrl->newcount[pp]) == 0) break;
+      const uint32_t qcount = ld_volatile(&ctrl->qc[par]);
+      ms_stage1<KW>(p, p.Q[par], qcount);
+      grid_barrier(&ctrl->bar, epoch);
+      if (blockIdx.x == 0 && threadIdx.x == 0) {
+        ctrl->qc[par] = 0;
+        ctrl->newcount[pp] = 0;
+      }
+      ms_stage2<KW>(p, sh, level, b0, nb, p.Q[par ^ 1u], &ctrl->qc[par ^ 1u], par);
+      grid_barrier(&ctrl->bar, epoch);
+    }
+  }
+}
+
+__global__ void closeness_finalize_kernel(uint32_t n, uint32_t rho, const uint32_t* perm, const unsigned long long* farT,
+                                          const uint32_t* reachT, const unsigned long long* farS, const uint32_t* reachS,
+                                          uint64_t nsrcs, double* cc, unsigned long long* farOut, uint32_t* reachOut) {
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nsrcs; i += (uint64_t)gridDim.x * blockDim.x) {
+    unsigned long long far;
+    uint32_t reach;
+    if (farT) {  // target-side sums (reading R13): source i = original vertex i
+      const uint32_t ui = perm ? perm[i] : (uint32_t)i;
+      const uint64_t idx = (uint64_t)(ui & 7u) * rho + (ui >> 3);
+      far = farT[idx];
+      reach = reachT[idx];
+    } else {
+      far = farS[i];
+      reach = reachS[i];
+    }
+    if (farOut) farOut[i] = far;
+    if (reachOut) reachOut[i] = reach;
+    // Eq. 8 with the component-size normalisation (reading R14): one IEEE fp64 division
+    if (cc) cc[i] = far == 0 ? 0.0 : (double)(reach - 1u) / (double)far;
+  }
+}
+
+template <class K>
+int coop_blocks(K kernel) {
+  int dev = 0, sms = 0, perSm = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&perSm, kernel, BLOCK_THREADS, 0) != cudaSuccess) return 0;
+  return sms * (perSm > 0 ? 1 : 0);
+}
+
+}  // namespace
+
+cudaError_t launch_msbfs(const MsParams& p, int gridBlocks, cudaStream_t st) {
+  void* args[] = {(void*)&p};
+  const void* k = nullptr;
+  switch (p.kappa) {
+    case 32: k = (const void*)msbfs_kernel<1>; break;
+    case 64: k = (const void*)msbfs_kernel<2>; break;
+    case 128: k = (const void*)msbfs_kernel<4>; break;
+    default: return cudaErrorInvalidValue;
+  }
+  return cudaLaunchCooperativeKernel(k, dim3(gridBlocks), dim3(BLOCK_THREADS), args, 0, st);
+}
+
+cudaError_t launch_closeness_finalize(uint32_t n, uint32_t rho, const uint32_t* perm, const unsigned long long* farT,
+                                      const uint32_t* reachT, const unsigned long long* farS, const uint32_t* reachS,
+                                      uint64_t nsrcs, double* cc, unsigned long long* farOut, uint32_t* reachOut,
+                                      cudaStream_t st) {
+  const int threads = 256;
+  const int blocks = (int)std::min<uint64_t>((nsrcs + threads - 1) / threads, 148ull * 8);
+  closeness_finalize_kernel<<<blocks > 0 ? blocks : 1, threads, 0, st>>>(n, rho, perm, farT, reachT, farS, reachS, nsrcs, cc,
+                                                                          farOut, reachOut);
+  return cudaGetLastError();
+}
+
+int max_coop_blocks_msbfs() { return coop_blocks(msbfs_kernel<4>); }
+
+}  // namespace blest

@@ -1,0 +1,257 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, bit-exact for levels,
+farness and reach; closeness within 1e-12 relative (expected bit-equal).  Sizes the oracle finishes in seconds, spanning
+several tiles, ragged tails and the degenerate cases.  Every path is forced in turn (policy independence, T5)."""
+import numpy as np
+import pytest
+
+import graphgen as gg
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def blest():
+    import paper_2606_05081_b200 as b
+
+    b.load()
+    return b
+
+
+SMALL = {
+    "path1000": lambda: gg.path(1000),                                  # ~1000 levels: persistent loop
+    "star_hub": lambda: gg.star(5000, 17),                              # one slice set with >> tau slices, hub row
+    "complete": lambda: gg.complete(130),
+    "union": lambda: gg.disjoint_union(gg.path(9), gg.empty(5), gg.complete(6), gg.cycle(11)),
+    "ragged": lambda: gg.gnm(1003, 2500, 7),                            # n not a multiple of 8 / 32 / 128
+    "grid": lambda: gg.grid2d(37, 41, 0.05, 8),
+    "rmat12": lambda: gg.rmat(12, 16, 9),
+    "tiny": lambda: gg.path(2),
+    "single": lambda: gg.empty(1),
+}
+
+
+def sources_for(n, rp, k=4):
+    deg = gg.degrees(rp)
+    s = {0, n - 1, int(np.argmax(deg))}
+    iso = np.flatnonzero(deg == 0)
+    if iso.size:
+        s.add(int(iso[0]))                                               # isolated source
+    s |= {int(x) for x in gg.pick_sources(rp, min(k, n), 5, nonzero_degree=False)}
+    return sorted(s)
+
+
+def check_bfs(blest, torch, g, graph, srcs, host_out=False):
+    n, rp, ci = graph
+    for s in srcs:
+        want = oracle.bfs(n, rp, ci, s)
+        if host_out:
+            out = np.full(n, 7, dtype=np.int32)
+            g.bfs(s, out)
+            torch.cuda.synchronize()
+            got = out
+        else:
+            out = torch.full((n,), 7, dtype=torch.int32, device="cuda")
+            g.bfs(s, out)
+            got = out.cpu().numpy()
+        assert np.array_equal(got, want), f"src {s}: {np.flatnonzero(got != want)[:8]}"
+        tr = g.trace()                                                   # also surfaces a queue overflow
+        assert len(tr) >= int(want.max())
+
+
+def test_contraction_forms_exhaustive(blest, torch_cuda):
+    """Every contraction form == (mask & alpha) != 0 over all 2^8 x 2^8 pairs in all four byte positions (T2)."""
+    for form in ("alu", "mma_b1", "mma_u8"):
+        assert blest.contraction_selftest(form) == 0, form
+
+
+@pytest.mark.parametrize("name", sorted(SMALL))
+@pytest.mark.parametrize("kernel", ["lazy", "eager"])
+def test_small_graphs_default_policy(blest, torch_cuda, name, kernel):
+    graph = SMALL[name]()
+    with blest.Graph(*graph, kernel=kernel) as g:
+        check_bfs(blest, torch_cuda, g, graph, sources_for(graph[0], graph[1]))
+
+
+@pytest.mark.parametrize("name", ["star_hub", "union", "ragged", "rmat12", "grid"])
+@pytest.mark.parametrize("switching", ["auto", "off", "bottom_up", "top_down", "slice"])
+def test_policy_independence_lazy(blest, torch_cuda, name, switching):
+    """Forcing each path on every level yields identical levels."""
+    graph = SMALL[name]()
+    with blest.Graph(*graph, kernel="lazy", switching=switching) as g:
+        check_bfs(blest, torch_cuda, g, graph, sources_for(graph[0], graph[1], 3))
+
+
+@pytest.mark.parametrize("mask", [0b10, 0b1100, 0b10101010, 0xFFFFFFF0])
+def test_scripted_direction_per_level(blest, torch_cuda, mask):
+    graph = SMALL["rmat12"]()
+    with blest.Graph(*graph, kernel="lazy", switching="scripted", bu_mask=mask) as g:
+        check_bfs(blest, torch_cuda, g, graph, sources_for(graph[0], graph[1], 2))
+        modes = g.trace()["mode"]
+        for lvl, m in enumerate(modes, start=1):
+            assert m == ((mask >> min(lvl, 31)) & 1)
+
+
+@pytest.mark.parametrize("contraction", ["alu", "mma_b1", "mma_u8"])
+@pytest.mark.parametrize("kernel", ["lazy", "eager"])
+def test_contraction_forms_in_traversal(blest, torch_cuda, contraction, kernel):
+    graph = SMALL["rmat12"]()
+    with blest.Graph(*graph, kernel=kernel, contraction=contraction, switching="off") as g:
+        check_bfs(blest, torch_cuda, g, graph, sources_for(graph[0], graph[1], 2))
+
+
+@pytest.mark.parametrize("reorder", ["none", "degree", "rcm"])
+@pytest.mark.parametrize("kernel", ["lazy", "eager"])
+def test_reordering_is_invisible(blest, torch_cuda, reorder, kernel):
+    for name in ("rmat12", "grid", "union"):
+        graph = SMALL[name]()
+        with blest.Graph(*graph, kernel=kernel, reorder=reorder, validate=True) as g:
+            check_bfs(blest, torch_cuda, g, graph, sources_for(graph[0], graph[1], 2))
+            check_bfs(blest, torch_cuda, g, graph, sources_for(graph[0], graph[1], 1)[:2], host_out=True)
+
+
+def test_device_csr_input_and_stream(blest, torch_cuda):
+    torch = torch_cuda
+    n, rp, ci = SMALL["rmat12"]()
+    drp = torch.from_numpy(rp.view(np.int32)).cuda()
+    dci = torch.from_numpy(ci.view(np.int32)).cuda()
+    st = torch.cuda.Stream()
+    with blest.Graph(n, drp, dci) as g:
+        out = torch.empty(n, dtype=torch.int32, device="cuda")
+        with torch.cuda.stream(st):
+            g.bfs(3, out, stream=st)
+        st.synchronize()
+        assert np.array_equal(out.cpu().numpy(), oracle.bfs(n, rp, ci, 3))
+
+
+def test_config1_rmat16_all_64_sources(blest, torch_cuda):
+    """BASELINE.json configs[0] at full size: RMAT scale 16, 64 seeded sources."""
+    torch = torch_cuda
+    n, rp, ci = gg.make_config("c1_rmat16")
+    srcs = gg.config_sources("c1_rmat16", rp)
+    assert srcs.size == 64
+    for opts in (dict(), dict(reorder="degree"), dict(kernel="eager"), dict(kernel="lazy", switching="off")):
+        with blest.Graph(n, rp, ci, **opts) as g:
+            out = torch.empty(n, dtype=torch.int32, device="cuda")
+            for s in srcs:
+                g.bfs(int(s), out)
+                assert np.array_equal(out.cpu().numpy(), oracle.bfs(n, rp, ci, int(s))), (opts, int(s))
+
+
+@pytest.mark.parametrize("name,shrink", [("c2_grid4096", 4), ("c3_gnm25", 7), ("c4_rmat24", 6), ("c5_rmat18", 2)])
+def test_configs_reduced(blest, torch_cuda, name, shrink):
+    torch = torch_cuda
+    n, rp, ci = gg.make_config(name, shrink)
+    srcs = gg.config_sources(name, rp)[:4] if name != "c5_rmat18" else gg.pick_sources(rp, 4, 3)
+    reorder = {"c4_rmat24": "degree", "c3_gnm25": "rcm"}.get(name, "none")
+    with blest.Graph(n, rp, ci, reorder=reorder) as g:
+        out = torch.empty(n, dtype=torch.int32, device="cuda")
+        for s in srcs:
+            g.bfs(int(s), out)
+            assert np.array_equal(out.cpu().numpy(), oracle.bfs(n, rp, ci, int(s)))
+
+
+# ---- multi-source BFS (A11) and closeness (A12) ------------------------------------------------------------------
+@pytest.mark.parametrize("kappa", [32, 64, 128])
+def test_msbfs_rows_equal_single_source(blest, torch_cuda, kappa):
+    torch = torch_cuda
+    graph = gg.disjoint_union(gg.rmat(9, 8, 11), gg.path(13), gg.empty(3))
+    n, rp, ci = graph
+    rng = np.random.Generator(np.random.PCG64(kappa))
+    with blest.Graph(n, rp, ci, kappa=kappa) as g:
+        for k in (1, kappa - 1, kappa, kappa + 1, 2 * kappa + 3):
+            srcs = rng.integers(0, n, size=k).astype(np.uint32)
+            if k >= 4:
+                srcs[1] = srcs[0]                                        # duplicate sources
+                srcs[2] = (srcs[0] & ~np.uint32(7)) | ((srcs[0] + 1) & 7)  # two sources sharing a slice set
+                srcs[3] = n - 1                                          # isolated vertex
+            want = oracle.msbfs(n, rp, ci, srcs)
+            out = torch.full((k, n), 9, dtype=torch.int32, device="cuda")
+            g.msbfs(srcs, out)
+            assert np.array_equal(out.cpu().numpy(), want), k
+            host = np.full((k, n), 9, dtype=np.int32)
+            g.msbfs(srcs, host)
+            assert np.array_equal(host, want)
+
+
+@pytest.mark.parametrize("reorder", ["none", "degree"])
+@pytest.mark.parametrize("kappa", [32, 64, 128])
+def test_closeness_all_vertices(blest, torch_cuda, reorder, kappa):
+    torch = torch_cuda
+    graph = gg.disjoint_union(gg.rmat(10, 8, 21), gg.star(30, 2), gg.empty(5), gg.path(2))
+    n, rp, ci = graph
+    far_w, reach_w, cc_w, _ = oracle.closeness(n, rp, ci)
+    with blest.Graph(n, rp, ci, kappa=kappa, reorder=reorder) as g:
+        far = torch.zeros(n, dtype=torch.int64, device="cuda")
+        reach = torch.zeros(n, dtype=torch.int32, device="cuda")
+        g.farness(far, reach)
+        assert np.array_equal(far.cpu().numpy().view(np.uint64), far_w)           # bit-exact integers
+        assert np.array_equal(reach.cpu().numpy().view(np.uint32), reach_w)
+        cc = torch.zeros(n, dtype=torch.float64, device="cuda")
+        g.closeness(cc)
+        got = cc.cpu().numpy()
+        assert np.allclose(got, cc_w, rtol=1e-12, atol=0.0) and np.array_equal(got == 0.0, cc_w == 0.0)
+        assert np.array_equal(got, cc_w)                                          # one IEEE division on both sides
+        host = np.zeros(n, dtype=np.float64)
+        g.closeness(host)
+        assert np.array_equal(host, cc_w)
+
+
+@pytest.mark.parametrize("kappa", [32, 64])
+def test_closeness_source_subset(blest, torch_cuda, kappa):
+    """Arbitrary source subsets use per-source counts (reading R13), incl. duplicates and k not a multiple of kappa."""
+    torch = torch_cuda
+    n, rp, ci = gg.disjoint_union(gg.rmat(9, 8, 31), gg.cycle(7), gg.empty(2))
+    srcs = np.array([5, 5, 0, n - 1, n - 4, 100, 17] + list(range(40, 40 + kappa)), dtype=np.uint32)
+    far_w, reach_w, cc_w, _ = oracle.closeness(n, rp, ci, srcs)
+    with blest.Graph(n, rp, ci, kappa=kappa) as g:
+        far = np.zeros(srcs.size, dtype=np.uint64)
+        reach = np.zeros(srcs.size, dtype=np.uint32)
+        g.farness(far, reach, srcs=srcs)
+        assert np.array_equal(far, far_w) and np.array_equal(reach, reach_w)
+        cc = torch.zeros(srcs.size, dtype=torch.float64, device="cuda")
+        g.closeness(cc, srcs=srcs)
+        assert np.array_equal(cc.cpu().numpy(), cc_w)
+
+
+def test_trace_and_info(blest, torch_cuda):
+    torch = torch_cuda
+    n, rp, ci = SMALL["rmat12"]()
+    with blest.Graph(n, rp, ci, kernel="lazy", reorder="degree") as g:
+        i = g.info()
+        assert i.n == n and i.nnz == ci.size and i.num_sms > 0 and i.grid_blocks == i.num_sms and i.kernel_chosen == 2
+        out = torch.empty(n, dtype=torch.int32, device="cuda")
+        s = int(gg.pick_sources(rp, 1, 1)[0])
+        g.bfs(s, out)
+        want = oracle.bfs(n, rp, ci, s)
+        tr = g.trace()
+        depth = int(want.max())
+        assert len(tr) == depth + 1                                      # the last level discovers nothing
+        for lvl in range(1, depth + 1):
+            assert tr["new_vertices"][lvl - 1] == np.count_nonzero(want == lvl)
+        assert tr["new_vertices"][-1] == 0 and np.all(np.diff(tr["t_ns"].astype(np.int64)) > 0)
+        assert tr["unvisited"][-1] == np.count_nonzero(want < 0)
+
+
+def test_bad_arguments(blest, torch_cuda):
+    from paper_2606_05081_b200 import binding
+
+    torch = torch_cuda
+    n, rp, ci = SMALL["union"]()
+    with blest.Graph(n, rp, ci) as g:
+        out = torch.empty(n, dtype=torch.int32, device="cuda")
+        with pytest.raises(blest.BlestError) as e:
+            g.bfs(n, out)
+        assert e.value.status == binding.EINVAL
+        with pytest.raises(blest.BlestError):
+            g.msbfs(np.array([n], np.uint32), torch.empty((1, n), dtype=torch.int32, device="cuda"))
+        with pytest.raises(blest.BlestError):
+            g.closeness(torch.empty(3, dtype=torch.float64, device="cuda"), srcs=np.array([0, 1, n + 5], np.uint32))
