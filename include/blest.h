@@ -102,6 +102,7 @@ typedef struct {
   uint32_t unvisited;   /* after this level */
   uint32_t reserved;
   uint64_t t_ns;        /* %globaltimer at the end of the level, relative to kernel start */
+  uint64_t t_stage1_ns; /* %globaltimer after the Stage-1 barrier of this level (lazy kernel), relative to kernel start */
 } blest_level_trace_t;
 
 /* Build: (optional reorder) -> BVSS -> U_div + dispatch -> upload.

@@ -60,12 +60,13 @@ class _Info(ctypes.Structure):
 class _Trace(ctypes.Structure):
     _fields_ = [("level", ctypes.c_uint32), ("mode", ctypes.c_uint32), ("q_entries", ctypes.c_uint32),
                 ("new_vertices", ctypes.c_uint32), ("q_bytes", ctypes.c_uint64), ("bu_scanned", ctypes.c_uint64),
-                ("unvisited", ctypes.c_uint32), ("reserved", ctypes.c_uint32), ("t_ns", ctypes.c_uint64)]
+                ("unvisited", ctypes.c_uint32), ("reserved", ctypes.c_uint32), ("t_ns", ctypes.c_uint64),
+                ("t_stage1_ns", ctypes.c_uint64)]
 
 
 TRACE_DTYPE = np.dtype([("level", "<u4"), ("mode", "<u4"), ("q_entries", "<u4"), ("new_vertices", "<u4"),
                         ("q_bytes", "<u8"), ("bu_scanned", "<u8"), ("unvisited", "<u4"), ("reserved", "<u4"),
-                        ("t_ns", "<u8")])
+                        ("t_ns", "<u8"), ("t_stage1_ns", "<u8")])
 
 EXPORTS = ["blest_build", "blest_preprocess_host", "blest_configure", "blest_bfs", "blest_msbfs", "blest_closeness", "blest_farness",
            "blest_get_info", "blest_get_trace", "blest_get_array", "blest_get_vi", "blest_contraction_selftest",

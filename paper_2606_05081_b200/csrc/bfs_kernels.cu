@@ -278,6 +278,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     if (bottomUp) stage1_bottom_up(p, sh, par);
     else stage1_queue<CONTR>(p, p.Q[par], qcount);
     grid_barrier(&ctrl->bar, epoch);
+    const unsigned long long tStage1 = (blockIdx.x == 0 && threadIdx.x == 0) ? globaltimer() : 0ull;
     // ---- Stage 2: frontier finalisation; counters consumed above are recycled here
     if (blockIdx.x == 0 && threadIdx.x == 0) {
       ctrl->qc[par] = 0;
@@ -300,6 +301,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       r.unvisited = (uint32_t)ld_volatile(&ctrl->unvisited[par]);
       r.reserved = 0;
       r.t_ns = globaltimer() - ctrl->t0;
+      r.t_stage1_ns = tStage1 - ctrl->t0;
       p.trace[level - 1] = r;
     }
   }
@@ -389,6 +391,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_eager_kernel(const __gri
       r.unvisited = 0;
       r.reserved = 0;
       r.t_ns = globaltimer() - ctrl->t0;
+      r.t_stage1_ns = r.t_ns;
       p.trace[level - 1] = r;
     }
   }
