@@ -131,19 +131,23 @@ def component_edges(deg: np.ndarray, levels: np.ndarray) -> int:
     return int(deg[levels >= 0].sum() // 2)
 
 
-def w_alg_bytes(trace: np.ndarray, n: int, reach: int, reordered: bool) -> int:
+def w_alg_bytes(trace: np.ndarray, n: int, reach: int, reordered: bool, sweep_words: int) -> int:
     """Algorithmic bytes of one blest_bfs launch, from the kernel's per-level trace:
-    queue levels: 8 B per queue entry + the graph bytes the entries cover (20 B per quad, 4 B per edge);
-    bottom-up levels: 4 B per neighbour scanned + 8 B of row pointers per unvisited vertex examined;
-    every level: the bitmap sweep 3 * n/8 B; per call: 4n B level init + 4 B per reached vertex (+ 4 B iperm)."""
-    w = 4 * n + (8 if reordered else 4) * reach
+    top-down levels: the graph bytes the frontier's work covers (20 B per quad of a slice set, 4 B per edge of a
+    frontier vertex) + 12 B per frontier word (list entry, frontier word, row pointers) + the finalisation sweep
+    (3 bitmap words per 32 vertices of the sweep range);
+    bottom-up levels: 4 B per neighbour scanned + 8 B of row pointers per unvisited vertex examined + the fused sweep
+    (3 bitmap words);
+    per call: 4 bitmap clears, 4 B level write per reached vertex; hand-off 4n B out (+ 4n B perm + 4 B per reached
+    vertex gathered, when the graph was reordered)."""
+    w = 16 * sweep_words + 4 * reach + 4 * n + ((4 * n + 4 * reach) if reordered else 0)
     unv_prev = n - 1
     for r in trace:
         if r["mode"] == 1:
-            w += 4 * int(r["bu_scanned"]) + 8 * unv_prev
+            w += 4 * int(r["bu_scanned"]) + 8 * min(unv_prev, 32 * sweep_words)
         else:
-            w += int(r["q_bytes"]) + 8 * int(r["q_entries"])
-        w += 3 * (n // 8)
+            w += int(r["q_bytes"]) + 12 * int(r["q_entries"])
+        w += 12 * sweep_words
         unv_prev = int(r["unvisited"])
     return int(w)
 
@@ -247,6 +251,7 @@ def main():
     host_out = torch.empty(n, dtype=torch.int32).pin_memory()
 
     # per-source numerators + algorithmic bytes from one untimed pass (also warm-up #0)
+    sweep_words = int(info.n_sweep_words)
     edges = np.zeros(len(srcs), dtype=np.int64)
     walg = np.zeros(len(srcs), dtype=np.int64)
     nlevels = np.zeros(len(srcs), dtype=np.int64)
@@ -258,7 +263,7 @@ def main():
             edges[i] = component_edges(deg, lv)
             tr = g.trace()
             nlevels[i] = len(tr)
-            walg[i] = w_alg_bytes(tr, n, int((lv >= 0).sum()), reorder != "none")
+            walg[i] = w_alg_bytes(tr, n, int((lv >= 0).sum()), reorder != "none", sweep_words)
 
     def one_step(dst, evs=None):
         for i, s in enumerate(srcs):

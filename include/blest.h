@@ -89,6 +89,8 @@ typedef struct {
   int kernel_chosen;       /* 1 eager | 2 lazy (after auto dispatch) */
   int reorder, kappa, num_sms, grid_blocks, block_threads;
   uint32_t queue_capacity; /* entries per work queue */
+  uint32_t n_sweep_words;  /* 32-vertex words (internal ids) that hold a vertex of non-zero degree: the range the
+                              lazy kernel's per-level sweeps cover */
 } blest_info_t;
 
 /* One record per BFS level of the most recent blest_bfs call (written by the persistent kernel). */

@@ -54,7 +54,7 @@ class _Info(ctypes.Structure):
                 ("build_seconds", ctypes.c_double), ("upload_seconds", ctypes.c_double),
                 ("kernel_chosen", ctypes.c_int), ("reorder", ctypes.c_int), ("kappa", ctypes.c_int),
                 ("num_sms", ctypes.c_int), ("grid_blocks", ctypes.c_int), ("block_threads", ctypes.c_int),
-                ("queue_capacity", ctypes.c_uint32)]
+                ("queue_capacity", ctypes.c_uint32), ("n_sweep_words", ctypes.c_uint32)]
 
 
 class _Trace(ctypes.Structure):
@@ -162,7 +162,7 @@ class Info:
     bvss_bytes: int; csr_bytes: int; workspace_bytes: int; mask_density: float; u_div: float
     reorder_seconds: float; build_seconds: float; upload_seconds: float
     kernel_chosen: int; reorder: int; kappa: int; num_sms: int; grid_blocks: int; block_threads: int
-    queue_capacity: int
+    queue_capacity: int; n_sweep_words: int
 
 
 class Graph:

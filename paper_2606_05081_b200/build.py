@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libblest.so")
-SOURCES = ["api.cu", "bfs_kernels.cu", "msbfs_kernels.cu", "microbench.cu", "host_graph.cpp"]
+SOURCES = ["api.cu", "bfs_lazy.cu", "bfs_eager.cu", "msbfs_kernels.cu", "microbench.cu", "host_graph.cpp"]
 HEADERS = ["device_common.cuh", "bfs_kernels.cuh", "host_graph.h", os.path.join("..", "..", "include", "blest.h")]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

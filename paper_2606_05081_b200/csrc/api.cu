@@ -46,7 +46,10 @@ struct blest_graph {
   uint32_t *dSetPtr = nullptr, *dRowIds = nullptr, *dMasks = nullptr, *dRowptr = nullptr, *dColidx = nullptr;
   uint32_t *dPerm = nullptr, *dIperm = nullptr;
   // single-source workspace
-  uint32_t *dVc = nullptr, *dVn = nullptr, *dF = nullptr;
+  uint32_t nSweepWords = 0, nIsoInSweep = 0, recCap = 0, chunkCap = 0;
+  std::vector<uint32_t> isoBits;  // host bitmap of zero-degree vertices (internal ids): such a source reaches nothing
+  uint32_t *dV = nullptr, *dF[3] = {nullptr, nullptr, nullptr}, *dWL[2] = {nullptr, nullptr};
+  uint4 *dRecs = nullptr, *dChunks = nullptr;
   uint2* dQ[2] = {nullptr, nullptr};
   Ctrl* dCtrl = nullptr;
   blest_level_trace_t* dTrace = nullptr;
@@ -198,6 +201,19 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
     g->nSlices = b.nSlices;
     g->nQuads = b.nQuads;
     g->nwords = (g->n + 31) / 32;
+    {  // sweep range of the lazy kernel: the 32-vertex words that hold a vertex of non-zero degree
+      g->isoBits.assign(g->nwords, 0u);
+      uint32_t last = 0;
+      bool any = false;
+      for (uint32_t u = 0; u < g->n; ++u) {
+        if (gcsr->rowptr[u + 1] == gcsr->rowptr[u]) g->isoBits[u >> 5] |= 1u << (u & 31u);
+        else { last = u; any = true; }
+      }
+      g->nSweepWords = any ? last / 32u + 1u : 0u;
+      uint32_t iso = 0;
+      for (uint32_t w = 0; w < g->nSweepWords; ++w) iso += (uint32_t)__builtin_popcount(g->isoBits[w]);
+      g->nIsoInSweep = iso;
+    }
     g->realPtrs.swap(b.realPtrs);
     g->virtualToReal.swap(b.virtualToReal);
     g->opt = opt;
@@ -240,9 +256,16 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
       const uint64_t qcap64 = (uint64_t)g->Nv + g->n + g->nnz / TD_CHUNK + 1024;
       if (qcap64 > 0xFFFFFFF0ull) return BLEST_ERANGE;
       g->qcap = (uint32_t)qcap64;
-      if ((rc = dev_alloc(g, &g->dVc, (uint64_t)g->nwords + 4, true))) return rc;
-      if ((rc = dev_alloc(g, &g->dVn, (uint64_t)g->nwords + 4, true))) return rc;
-      if ((rc = dev_alloc(g, &g->dF, (uint64_t)g->nwords + 4, true))) return rc;
+      if ((rc = dev_alloc(g, &g->dV, (uint64_t)g->nwords + 4, true))) return rc;
+      for (int k = 0; k < 3; ++k)
+        if ((rc = dev_alloc(g, &g->dF[k], (uint64_t)g->nwords + 4, true))) return rc;
+      for (int k = 0; k < 2; ++k)
+        if ((rc = dev_alloc(g, &g->dWL[k], (uint64_t)g->nSweepWords + 16384))) return rc;
+      // every deferred segment owns more than BIG_EDGES edges / BIG_QUADS quads of its own => exact capacity bounds
+      g->recCap = (uint32_t)(g->nnz / BIG_EDGES + g->nQuads / BIG_QUADS + 16);
+      g->chunkCap = (uint32_t)(g->nnz / CHUNK_EDGES + g->nQuads / CHUNK_QUADS + g->recCap + 16);
+      if ((rc = dev_alloc(g, &g->dRecs, g->recCap))) return rc;
+      if ((rc = dev_alloc(g, &g->dChunks, g->chunkCap))) return rc;
       if ((rc = dev_alloc(g, &g->dQ[0], g->qcap))) return rc;
       if ((rc = dev_alloc(g, &g->dQ[1], g->qcap))) return rc;
       if ((rc = dev_alloc(g, &g->dCtrl, 1, true))) return rc;
@@ -271,6 +294,7 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
     I.grid_blocks = g->gridLazy;
     I.block_threads = BLOCK_THREADS;
     I.queue_capacity = g->qcap;
+    I.n_sweep_words = g->nSweepWords;
   } catch (const std::bad_alloc&) {
     return BLEST_ENOMEM;
   }
@@ -323,8 +347,13 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
   BfsParams p{};
   p.n = h->n; p.Ns = h->Ns; p.nwords = h->nwords; p.qcap = h->qcap; p.nnz = h->nnz;
   p.setPtr = h->dSetPtr; p.rowIds = reinterpret_cast<const uint4*>(h->dRowIds); p.masks = h->dMasks;
-  p.rowptr = h->dRowptr; p.colidx = h->dColidx; p.iperm = h->hasPerm ? h->dIperm : nullptr;
-  p.Vcurr = h->dVc; p.Vnext = h->dVn; p.Fcurr = h->dF;
+  p.rowptr = h->dRowptr; p.colidx = h->dColidx;
+  p.perm = h->hasPerm ? h->dPerm : nullptr;
+  p.iperm = h->hasPerm ? h->dIperm : nullptr;
+  p.nSweepWords = h->nSweepWords; p.nIsoInSweep = h->nIsoInSweep;
+  p.V = h->dV; p.F[0] = h->dF[0]; p.F[1] = h->dF[1]; p.F[2] = h->dF[2];
+  p.WL[0] = h->dWL[0]; p.WL[1] = h->dWL[1];
+  p.recs = h->dRecs; p.chunks = h->dChunks; p.recCap = h->recCap; p.chunkCap = h->chunkCap;
   p.Q[0] = h->dQ[0]; p.Q[1] = h->dQ[1];
   p.out = devOut ? levels_out : h->dOut;
   p.L = h->hasPerm ? h->dL : p.out;
@@ -339,7 +368,8 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
   p.eta = h->opt.eta;
   p.gamma = h->opt.gamma;
   CK(cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st));
-  if (resolved_kernel(h) == 1) CK(launch_bfs_eager(p, h->gridEager, st));
+  if ((h->isoBits[p.src >> 5] >> (p.src & 31u)) & 1u) CK(launch_isolated_source(p.out, h->n, src, st));  // nothing to traverse
+  else if (resolved_kernel(h) == 1) CK(launch_bfs_eager(p, h->gridEager, st));
   else CK(launch_bfs_lazy(p, h->gridLazy, st));
   if (!devOut) CK(cudaMemcpyAsync(levels_out, h->dOut, (size_t)h->n * 4, cudaMemcpyDeviceToHost, st));
   return BLEST_OK;

@@ -4,6 +4,14 @@
 
 namespace blest {
 
+// Tunables of the lazy kernel's top-down stage.
+constexpr uint32_t TINY_DEG = 8;        // edges of a frontier vertex scanned by its own lane
+constexpr uint32_t BIG_EDGES = 4096;    // longer adjacency lists are deferred to the balanced phase
+constexpr uint32_t BIG_QUADS = 1024;    // longer slice sets (in quads) are deferred to the balanced phase
+constexpr uint32_t CHUNK_EDGES = 1024;  // balanced phase: edges per chunk entry
+constexpr uint32_t CHUNK_QUADS = 256;   // balanced phase: quads per chunk entry
+constexpr uint32_t WL_STAGE = 4096;     // per-CTA shared-memory staging of frontier word ids
+
 struct BfsParams {
   // graph (immutable during traversal)
   uint32_t n, Ns, nwords, qcap;
@@ -13,15 +21,23 @@ struct BfsParams {
   const uint32_t* masks;   // nQuads
   const uint32_t* rowptr;  // internal (reordered) CSR, n+1
   const uint32_t* colidx;
+  const uint32_t* perm;    // original -> internal id, or nullptr when no reordering
   const uint32_t* iperm;   // internal -> original id, or nullptr when no reordering
-  // state
-  uint32_t* Vcurr;
-  uint32_t* Vnext;
-  uint32_t* Fcurr;
+  // lazy kernel state
+  uint32_t nSweepWords;    // 32-vertex words covering every vertex of non-zero degree
+  uint32_t nIsoInSweep;    // zero-degree vertices inside the sweep range
+  uint32_t* V;             // visited bitmap (single copy)
+  uint32_t* F[3];          // frontier bitmaps, rotating: level l reads F[(l-1)%3], writes F[l%3], clears F[(l+1)%3]
+  uint32_t* WL[2];         // frontier word lists (ids of non-zero words of the frontier bitmap), level parity
+  uint4* recs;             // deferred big segments {start, count, (set << 1) | type, first chunk}
+  uint4* chunks;           // balanced-phase chunk entries {start, count, set, type}
+  uint32_t recCap, chunkCap;
+  // eager kernel state
   uint2* Q[2];
+  int32_t* stamp;  // last level at which a slice set was enqueued
+  // levels
   int32_t* out;    // levels in ORIGINAL ids (device)
-  int32_t* L;      // eager: levels in internal ids (== out when iperm == nullptr)
-  int32_t* stamp;  // eager: last level at which a slice set was enqueued
+  int32_t* L;      // levels in internal ids (== out when there is no reordering)
   Ctrl* ctrl;
   blest_level_trace_t* trace;
   uint32_t traceCap;
@@ -58,6 +74,7 @@ struct MsParams {
 
 cudaError_t launch_bfs_lazy(const BfsParams& p, int gridBlocks, cudaStream_t st);
 cudaError_t launch_bfs_eager(const BfsParams& p, int gridBlocks, cudaStream_t st);
+cudaError_t launch_isolated_source(int32_t* out, uint32_t n, uint32_t src, cudaStream_t st);
 cudaError_t launch_msbfs(const MsParams& p, int gridBlocks, cudaStream_t st);
 cudaError_t launch_closeness_finalize(uint32_t n, uint32_t rho, const uint32_t* perm, const unsigned long long* farT,
                                       const uint32_t* reachT, const unsigned long long* farS, const uint32_t* reachS,

@@ -22,12 +22,14 @@ struct Ctrl {
   unsigned int nlevels;
   unsigned int pad0;
   unsigned int qc[4];               // work-queue entry counters (rotating)
-  unsigned long long qbytes[4];     // graph bytes covered by the entries of each queue
-  unsigned long long unvisited[2];  // per level parity
-  unsigned long long newcount[2];
-  unsigned long long mf[2];         // sum of degrees of the vertices discovered at this level
-  unsigned long long buScanned[2];  // neighbours scanned by the bottom-up stage
+  unsigned long long qbytes[4];     // graph bytes covered by the work of each level (rotating)
+  unsigned long long unvisited[4];  // per level (rotating)
+  unsigned long long newcount[4];
+  unsigned long long mf[4];         // sum of degrees of the vertices discovered at this level
+  unsigned long long buScanned[4];  // neighbours scanned by the bottom-up stage
   unsigned long long t0;            // %globaltimer at kernel start
+  unsigned int wlc[4];              // lazy kernel: frontier word-list lengths (rotating, level mod 3)
+  unsigned int nBig[4];             // lazy kernel: deferred big segments of the level (rotating)
 };
 
 __device__ __forceinline__ unsigned long long globaltimer() {
