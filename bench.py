@@ -132,23 +132,21 @@ def component_edges(deg: np.ndarray, levels: np.ndarray) -> int:
 
 
 def w_alg_bytes(trace: np.ndarray, n: int, reach: int, reordered: bool, sweep_words: int) -> int:
-    """Algorithmic bytes of one blest_bfs launch, from the kernel's per-level trace:
-    top-down levels: the graph bytes the frontier's work covers (20 B per quad of a slice set, 4 B per edge of a
-    frontier vertex) + 12 B per frontier word (list entry, frontier word, row pointers) + the finalisation sweep
-    (3 bitmap words per 32 vertices of the sweep range);
-    bottom-up levels: 4 B per neighbour scanned + 8 B of row pointers per unvisited vertex examined + the fused sweep
-    (3 bitmap words);
-    per call: 4 bitmap clears, 4 B level write per reached vertex; hand-off 4n B out (+ 4n B perm + 4 B per reached
-    vertex gathered, when the graph was reordered)."""
-    w = 16 * sweep_words + 4 * reach + 4 * n + ((4 * n + 4 * reach) if reordered else 0)
-    unv_prev = n - 1
+    """Algorithmic bytes of one blest_bfs launch, from the kernel's own per-level trace.
+    per call:   4 bitmaps cleared (16 B per sweep word) + levels_out pre-filled with -1 (4n B);
+    every level: `q_bytes` = the graph bytes its work items cover (top-down: 20 B per quad of a slice work item, 4 B per
+                CSR edge + 8 B of row pointers per edge work item; bottom-up: 8 B inline head per unvisited vertex examined,
+                8 B of row pointers + 4 B per neighbour for the vertices that need the CSR scan);
+                top-down adds 12 B per frontier word consumed (list entry, frontier word, threshold) and the finalisation
+                sweep (12 B per sweep word: V, F_next read, F_stale cleared); bottom-up adds its sweep (8 B per sweep word);
+    per discovered vertex: 4 B level write + 4 B degree (+ 4 B iperm when the graph was reordered)."""
+    w = 16 * sweep_words + 4 * n + reach * (12 if reordered else 8)
     for r in trace:
+        w += int(r["q_bytes"])
         if r["mode"] == 1:
-            w += 4 * int(r["bu_scanned"]) + 8 * min(unv_prev, 32 * sweep_words)
+            w += 8 * sweep_words
         else:
-            w += int(r["q_bytes"]) + 12 * int(r["q_entries"])
-        w += 12 * sweep_words
-        unv_prev = int(r["unvisited"])
+            w += 12 * int(r["q_entries"]) + 12 * sweep_words
     return int(w)
 
 

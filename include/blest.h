@@ -63,14 +63,16 @@ typedef struct {
   int kernel;      /* 0 auto by U_div | 1 eager (Alg. 2) | 2 lazy two-stage (Alg. 3) */
   int switching;   /* 0 auto (per-level cost model; Eq. 6 analogue) | 1 off: slice path only |
                       2 force bottom-up CUDA-core (Alg. 4) on every level >= 2 |
-                      3 force top-down CUDA-core (CSR edge chunks) | 4 force slice path */
+                      3 force top-down CUDA-core (CSR edges) | 4 force slice path | 5 scripted (reserved[0]) */
   int contraction; /* 0 auto | 1 ALU (AND + per-byte test) | 2 mma.sync m8n8k128 b1 and.popc (paper layout, Fig. 3) |
                       3 mma.sync m16n8k32 u8 (bits expanded to bytes) */
   int kappa;       /* multi-source width: 0 -> 64 | 32 | 64 | 128 (reading R19) */
   int trace;       /* 0 | 1: keep the per-level trace (always cheap; default on) */
   float eta;       /* bottom-up switch constant (Eq. 6, eta = 10 on Hopper); 0 -> library default */
-  float gamma;     /* slice-vs-edge-chunk byte ratio for the per-slice-set top-down choice; 0 -> default */
-  int reserved[6];
+  float gamma;     /* scales the slice-path cost in the per-slice-set slice-vs-CSR-edges threshold; 0 -> 1.0 */
+  int reserved[6]; /* [0]: switching == 5 ("scripted", tests): level l runs bottom-up iff bit min(l,31) is set;
+                      [1..5]: tuning overrides of the switch cost model in 0.01 ps per unit (top-down edge, top-down
+                      vertex, bottom-up vertex, bottom-up scanned neighbour, bottom-up bitmap word); 0 = default */
 } blest_options_t;
 
 typedef struct {
@@ -142,6 +144,11 @@ int blest_get_info(blest_handle_t h, blest_info_t *info);
 /* Per-level trace of the last blest_bfs call.  Synchronises the device.  *n_levels = records available
  * (may exceed cap; only min(cap, available) are copied). */
 int blest_get_trace(blest_handle_t h, blest_level_trace_t *buf, uint32_t cap, uint32_t *n_levels);
+
+/* Timing of the most recent blest_bfs call on the lazy kernel, from the kernel's own %globaltimer stamps:
+ * *init_ns = kernel start -> end of the per-call init (bitmap clears, levels_out = -1), *levels_ns = kernel start ->
+ * end of the last level.  Synchronises the device.  Either pointer may be NULL. */
+int blest_get_call_stats(blest_handle_t h, uint64_t *init_ns, uint64_t *levels_ns);
 
 /* Copy one internal array to a HOST buffer (tests: BVSS round trip, permutation bijection).  `which`:
  * 0 setPtr uint32[N_s+1] (quad offsets) | 1 rowIds uint32[4*n_quads] | 2 masks uint32[n_quads] |

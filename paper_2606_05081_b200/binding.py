@@ -68,7 +68,7 @@ TRACE_DTYPE = np.dtype([("level", "<u4"), ("mode", "<u4"), ("q_entries", "<u4"),
                         ("q_bytes", "<u8"), ("bu_scanned", "<u8"), ("unvisited", "<u4"), ("reserved", "<u4"),
                         ("t_ns", "<u8"), ("t_stage1_ns", "<u8")])
 
-EXPORTS = ["blest_build", "blest_preprocess_host", "blest_configure", "blest_bfs", "blest_msbfs", "blest_closeness", "blest_farness",
+EXPORTS = ["blest_build", "blest_preprocess_host", "blest_configure", "blest_get_call_stats", "blest_bfs", "blest_msbfs", "blest_closeness", "blest_farness",
            "blest_get_info", "blest_get_trace", "blest_get_array", "blest_get_vi", "blest_contraction_selftest",
            "blest_mma_microbench", "blest_barrier_microbench", "blest_destroy", "blest_strerror",
            "blest_last_cuda_error"]
@@ -94,6 +94,7 @@ def load(build_if_missing: bool = True):
     L.blest_farness.argtypes = [vp, vp, u64, vp, vp, vp]
     L.blest_get_info.argtypes = [vp, ctypes.POINTER(_Info)]
     L.blest_get_trace.argtypes = [vp, vp, u32, ctypes.POINTER(u32)]
+    L.blest_get_call_stats.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
     L.blest_get_array.argtypes = [vp, i32, vp, u64]
     L.blest_get_vi.argtypes = [u64, u64]
     L.blest_get_vi.restype = u64
@@ -140,7 +141,7 @@ def _stream(stream):
 
 
 def _options(reorder="none", builder=0, validate=False, kernel="auto", switching="auto", contraction="auto", kappa=64,
-             trace=True, eta=0.0, gamma=0.0, bu_mask=0) -> _Options:
+             trace=True, eta=0.0, gamma=0.0, bu_mask=0, costs=None) -> _Options:
     o = _Options()
     o.reorder = REORDER[reorder] if isinstance(reorder, str) else int(reorder)
     o.builder = int(builder)
@@ -153,6 +154,8 @@ def _options(reorder="none", builder=0, validate=False, kernel="auto", switching
     o.eta = float(eta)
     o.gamma = float(gamma)
     o.reserved[0] = int(bu_mask)
+    for k, c in enumerate(costs or ()):  # switch cost model overrides, ps per unit (tuning only): td_edge, td_vertex,
+        o.reserved[1 + k] = int(round(100 * float(c)))  # bu_vertex, bu_scan, bu_word
     return o
 
 
@@ -246,6 +249,12 @@ class Graph:
         i = _Info()
         _check(load().blest_get_info(self._h, ctypes.byref(i)), "blest_get_info")
         return Info(**{f[0]: getattr(i, f[0]) for f in _Info._fields_})
+
+    def call_stats(self):
+        """(init_ns, levels_ns) of the last bfs call on the lazy kernel."""
+        a, b = ctypes.c_uint64(0), ctypes.c_uint64(0)
+        _check(load().blest_get_call_stats(self._h, ctypes.byref(a), ctypes.byref(b)), "blest_get_call_stats")
+        return int(a.value), int(b.value)
 
     def trace(self) -> np.ndarray:
         """Per-level records of the last bfs() call (structured array, TRACE_DTYPE).  Synchronises the device."""

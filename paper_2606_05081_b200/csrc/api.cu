@@ -30,6 +30,9 @@ static thread_local int g_lastCuda = 0;
 
 static constexpr uint32_t TRACE_CAP = 1u << 17;
 static constexpr double UDIV_THRESHOLD = 25000.0;
+// switch cost model defaults, picoseconds per unit
+static constexpr float COST_TD_EDGE = 8.0f, COST_TD_VERTEX = 40.0f, COST_TD_WORD = 30.0f;
+static constexpr float COST_BU_VERTEX = 4.0f, COST_BU_SCAN = 6.0f, COST_BU_WORD = 20.0f;
 
 struct blest_graph {
   uint32_t n = 0, Ns = 0, Nv = 0, nwords = 0, rho = 0, qcap = 0;
@@ -46,10 +49,15 @@ struct blest_graph {
   uint32_t *dSetPtr = nullptr, *dRowIds = nullptr, *dMasks = nullptr, *dRowptr = nullptr, *dColidx = nullptr;
   uint32_t *dPerm = nullptr, *dIperm = nullptr;
   // single-source workspace
-  uint32_t nSweepWords = 0, nIsoInSweep = 0, recCap = 0, chunkCap = 0;
+  uint32_t nSweepWords = 0, nIsoInSweep = 0, chunkCap = 0;
+  std::vector<uint32_t> setQuads;  // per slice set: quads stored          (popThr is rebuilt when gamma changes)
+  std::vector<uint64_t> setDeg;    // per slice set: degree sum of its 8 columns
+  uint2* dHead = nullptr;
+  uint32_t* dDeg = nullptr;
+  uint16_t* dPopThr = nullptr;
   std::vector<uint32_t> isoBits;  // host bitmap of zero-degree vertices (internal ids): such a source reaches nothing
   uint32_t *dV = nullptr, *dF[3] = {nullptr, nullptr, nullptr}, *dWL[2] = {nullptr, nullptr};
-  uint4 *dRecs = nullptr, *dChunks = nullptr;
+  uint4* dChunks = nullptr;
   uint2* dQ[2] = {nullptr, nullptr};
   Ctrl* dCtrl = nullptr;
   blest_level_trace_t* dTrace = nullptr;
@@ -97,6 +105,41 @@ static int check_options(const blest_options_t& o) {
   if (o.kernel < 0 || o.kernel > 2 || o.switching < 0 || o.switching > 5) return BLEST_EINVAL;
   if (o.contraction < 0 || o.contraction > 3) return BLEST_EINVAL;
   if (o.kappa != 0 && o.kappa != 32 && o.kappa != 64 && o.kappa != 128) return BLEST_EINVAL;
+  return BLEST_OK;
+}
+
+// Per slice set: the smallest number k of frontier columns from which the slice path is expected to be cheaper than
+// the CSR edges of those columns.  Costs in byte equivalents; a bitmap probe / mark counts as MARK
+// bytes (one 32-byte L2 sector request).  Slices: 20 B per quad + one mark per slice that hits,
+// P(hit) = 1 - (1 - k/8)^rho with rho = edges per slice; edges: (k/8) of the set's edges, 4 B + one mark each.
+static void build_pop_thresholds(const blest_graph* g, float gamma, std::vector<uint16_t>& thr) {
+  constexpr double MARK = 32.0;
+  thr.assign(g->nwords, 0x9999u);
+#pragma omp parallel for schedule(static)
+  for (int64_t w = 0; w < (int64_t)g->nwords; ++w) {
+    uint32_t packed = 0;
+    for (uint32_t q = 0; q < 4; ++q) {
+      const uint64_t s = (uint64_t)w * 4 + q;
+      uint32_t t = 9;
+      if (s < g->Ns && g->setQuads[s] > 0 && g->setDeg[s] > 0) {
+        const double nq = g->setQuads[s], D = (double)g->setDeg[s];
+        const double S = 4.0 * nq, rho = std::max(1.0, D / S);
+        for (uint32_t k = 1; k <= 8; ++k) {
+          const double cs = 20.0 * nq + S * MARK * (1.0 - std::pow(1.0 - k / 8.0, rho));
+          const double ce = (k / 8.0) * D * (4.0 + MARK) + 8.0 * k;
+          if (cs * gamma <= ce) { t = k; break; }
+        }
+      }
+      packed |= t << (4 * q);
+    }
+    thr[w] = (uint16_t)packed;
+  }
+}
+
+static int upload_pop_thresholds(blest_graph* g) {
+  std::vector<uint16_t> thr;
+  build_pop_thresholds(g, g->opt.gamma, thr);
+  CK(cudaMemcpy(g->dPopThr, thr.data(), thr.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
   return BLEST_OK;
 }
 
@@ -249,6 +292,35 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
         CK(cudaMemcpy(g->dPerm, g->perm.data(), (size_t)g->n * 4, cudaMemcpyHostToDevice));
         CK(cudaMemcpy(g->dIperm, g->iperm.data(), (size_t)g->n * 4, cudaMemcpyHostToDevice));
       }
+      {  // auxiliary arrays of the CUDA-core paths: inline heads (first two neighbours), capped degrees, per-set
+         // degree sums for the slice/edge thresholds
+        std::vector<uint2> head(g->n);
+        std::vector<uint32_t> deg(g->n);
+#pragma omp parallel for schedule(static)
+        for (int64_t u = 0; u < (int64_t)g->n; ++u) {
+          const uint32_t b0 = gcsr->rowptr[u], d = gcsr->rowptr[u + 1] - b0;
+          uint2 hd = make_uint2(0xFFFFFFFFu, 0xFFFFFFFFu);
+          if (d >= 1) hd.x = gcsr->colidx[b0];
+          if (d >= 2) hd.y = gcsr->colidx[b0 + 1] | (d > 2 ? 0x80000000u : 0u);
+          head[u] = hd;
+          deg[u] = d;
+        }
+        g->setQuads.resize(g->Ns);
+        g->setDeg.resize(g->Ns);
+#pragma omp parallel for schedule(static)
+        for (int64_t s = 0; s < (int64_t)g->Ns; ++s) {
+          g->setQuads[s] = b.setPtr[s + 1] - b.setPtr[s];
+          const uint64_t u0 = (uint64_t)s * SIGMA, u1 = std::min<uint64_t>(u0 + SIGMA, g->n);
+          g->setDeg[s] = gcsr->rowptr[u1] - gcsr->rowptr[u0];
+        }
+        if ((rc = dev_alloc(g, &g->dHead, g->n))) return rc;
+        if ((rc = dev_alloc(g, &g->dDeg, g->n))) return rc;
+        if ((rc = dev_alloc(g, &g->dPopThr, (uint64_t)g->nwords + 16))) return rc;
+        CK(cudaMemcpy(g->dHead, head.data(), (size_t)g->n * sizeof(uint2), cudaMemcpyHostToDevice));
+        CK(cudaMemcpy(g->dDeg, deg.data(), (size_t)g->n * 4, cudaMemcpyHostToDevice));
+        g->info.csr_bytes += (uint64_t)g->n * 12 + (uint64_t)g->nwords * 2;
+        if ((rc = upload_pop_thresholds(g))) return rc;
+      }
       g->info.upload_seconds = now_s() - t0;
       { HostBvss drop; std::swap(drop, b); }  // release the host copy
 
@@ -256,15 +328,13 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
       const uint64_t qcap64 = (uint64_t)g->Nv + g->n + g->nnz / TD_CHUNK + 1024;
       if (qcap64 > 0xFFFFFFF0ull) return BLEST_ERANGE;
       g->qcap = (uint32_t)qcap64;
-      if ((rc = dev_alloc(g, &g->dV, (uint64_t)g->nwords + 4, true))) return rc;
+      if ((rc = dev_alloc(g, &g->dV, (uint64_t)g->nwords + 16, true))) return rc;
       for (int k = 0; k < 3; ++k)
-        if ((rc = dev_alloc(g, &g->dF[k], (uint64_t)g->nwords + 4, true))) return rc;
+        if ((rc = dev_alloc(g, &g->dF[k], (uint64_t)g->nwords + 16, true))) return rc;
       for (int k = 0; k < 2; ++k)
         if ((rc = dev_alloc(g, &g->dWL[k], (uint64_t)g->nSweepWords + 16384))) return rc;
       // every deferred segment owns more than BIG_EDGES edges / BIG_QUADS quads of its own => exact capacity bounds
-      g->recCap = (uint32_t)(g->nnz / BIG_EDGES + g->nQuads / BIG_QUADS + 16);
-      g->chunkCap = (uint32_t)(g->nnz / CHUNK_EDGES + g->nQuads / CHUNK_QUADS + g->recCap + 16);
-      if ((rc = dev_alloc(g, &g->dRecs, g->recCap))) return rc;
+      g->chunkCap = (uint32_t)(g->nnz / CHUNK_EDGES + g->nQuads / CHUNK_QUADS + g->nnz / BIG_EDGES + g->nQuads / BIG_QUADS + 16);
       if ((rc = dev_alloc(g, &g->dChunks, g->chunkCap))) return rc;
       if ((rc = dev_alloc(g, &g->dQ[0], g->qcap))) return rc;
       if ((rc = dev_alloc(g, &g->dQ[1], g->qcap))) return rc;
@@ -320,7 +390,9 @@ int blest_configure(blest_handle_t h, const blest_options_t* optIn) {
   int rc = check_options(o);
   if (rc) return rc;
   normalise_options(o);
+  const bool gammaChanged = o.gamma != h->opt.gamma;
   h->opt = o;
+  if (gammaChanged && !h->hostOnly) return upload_pop_thresholds(h);
   return BLEST_OK;
 }
 
@@ -353,7 +425,8 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
   p.nSweepWords = h->nSweepWords; p.nIsoInSweep = h->nIsoInSweep;
   p.V = h->dV; p.F[0] = h->dF[0]; p.F[1] = h->dF[1]; p.F[2] = h->dF[2];
   p.WL[0] = h->dWL[0]; p.WL[1] = h->dWL[1];
-  p.recs = h->dRecs; p.chunks = h->dChunks; p.recCap = h->recCap; p.chunkCap = h->chunkCap;
+  p.chunks = h->dChunks; p.chunkCap = h->chunkCap;
+  p.head = h->dHead; p.deg = h->dDeg; p.popThr = h->dPopThr;
   p.Q[0] = h->dQ[0]; p.Q[1] = h->dQ[1];
   p.out = devOut ? levels_out : h->dOut;
   p.L = h->hasPerm ? h->dL : p.out;
@@ -362,6 +435,13 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
   p.trace = h->opt.trace == 0 || h->opt.trace == 1 ? h->dTrace : nullptr;
   p.traceCap = TRACE_CAP;
   p.src = h->hasPerm ? h->perm[src] : src;
+  p.srcOrig = src;
+  {  // switch cost model, ps per unit (fitted to per-level traces on the B200); reserved[1..5] override (x0.01)
+    const float dflt[5] = {COST_TD_EDGE, COST_TD_VERTEX, COST_BU_VERTEX, COST_BU_SCAN, COST_BU_WORD};
+    float* dst[5] = {&p.cTdEdge, &p.cTdVertex, &p.cBuVertex, &p.cBuScan, &p.cBuWord};
+    for (int k = 0; k < 5; ++k) *dst[k] = h->opt.reserved[1 + k] > 0 ? 0.01f * (float)h->opt.reserved[1 + k] : dflt[k];
+    p.cTdWord = COST_TD_WORD;
+  }
   p.switching = h->opt.switching;
   p.contraction = h->opt.contraction ? h->opt.contraction : 1;  // auto -> ALU (measured fastest)
   p.buMask = (uint32_t)h->opt.reserved[0];
@@ -385,6 +465,24 @@ int blest_get_trace(blest_handle_t h, blest_level_trace_t* buf, uint32_t cap, ui
   const uint32_t k = std::min(std::min(cap, c.nlevels), TRACE_CAP);
   if (buf && k) CK(cudaMemcpy(buf, h->dTrace, (size_t)k * sizeof(blest_level_trace_t), cudaMemcpyDeviceToHost));
   return (c.error & 1u) ? BLEST_EOVERFLOW : BLEST_OK;
+}
+
+int blest_get_call_stats(blest_handle_t h, uint64_t* init_ns, uint64_t* levels_ns) {
+  if (!h) return BLEST_EINVAL;
+  if (h->hostOnly) return BLEST_EUNSUPPORTED;
+  CK(cudaDeviceSynchronize());
+  Ctrl c;
+  CK(cudaMemcpy(&c, h->dCtrl, sizeof(Ctrl), cudaMemcpyDeviceToHost));
+  if (init_ns) *init_ns = c.tInit;
+  if (levels_ns) {
+    *levels_ns = 0;
+    if (c.nlevels) {
+      blest_level_trace_t last;
+      CK(cudaMemcpy(&last, h->dTrace + std::min(c.nlevels, TRACE_CAP) - 1, sizeof(last), cudaMemcpyDeviceToHost));
+      *levels_ns = last.t_ns;
+    }
+  }
+  return BLEST_OK;
 }
 
 static int ensure_ms_workspace(blest_graph* g) {

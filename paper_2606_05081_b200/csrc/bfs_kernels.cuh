@@ -5,11 +5,10 @@
 namespace blest {
 
 // Tunables of the lazy kernel's top-down stage.
-constexpr uint32_t TINY_DEG = 8;        // edges of a frontier vertex scanned by its own lane
-constexpr uint32_t BIG_EDGES = 4096;    // longer adjacency lists are deferred to the balanced phase
-constexpr uint32_t BIG_QUADS = 1024;    // longer slice sets (in quads) are deferred to the balanced phase
-constexpr uint32_t CHUNK_EDGES = 1024;  // balanced phase: edges per chunk entry
-constexpr uint32_t CHUNK_QUADS = 256;   // balanced phase: quads per chunk entry
+constexpr uint32_t BIG_EDGES = 512;     // longer adjacency lists are deferred to the balanced phase
+constexpr uint32_t BIG_QUADS = 128;     // longer slice sets (in quads) are deferred to the balanced phase
+constexpr uint32_t CHUNK_EDGES = 256;   // balanced phase: edges per chunk entry
+constexpr uint32_t CHUNK_QUADS = 64;    // balanced phase: quads per chunk entry
 constexpr uint32_t WL_STAGE = 4096;     // per-CTA shared-memory staging of frontier word ids
 
 struct BfsParams {
@@ -23,15 +22,18 @@ struct BfsParams {
   const uint32_t* colidx;
   const uint32_t* perm;    // original -> internal id, or nullptr when no reordering
   const uint32_t* iperm;   // internal -> original id, or nullptr when no reordering
+  const uint2* head;       // n: first two neighbours of every vertex (x, y); 0xFFFFFFFF = none; y bit 31 = "has more"
+  const uint32_t* deg;     // n: degrees (read where a discovered vertex is finalised, for the switch counters)
+  const uint16_t* popThr;  // nwords: four 4-bit thresholds, one per slice set of the word (slice path iff
+                           // popc(frontier byte) >= threshold; 9 = never)
   // lazy kernel state
   uint32_t nSweepWords;    // 32-vertex words covering every vertex of non-zero degree
   uint32_t nIsoInSweep;    // zero-degree vertices inside the sweep range
   uint32_t* V;             // visited bitmap (single copy)
   uint32_t* F[3];          // frontier bitmaps, rotating: level l reads F[(l-1)%3], writes F[l%3], clears F[(l+1)%3]
   uint32_t* WL[2];         // frontier word lists (ids of non-zero words of the frontier bitmap), level parity
-  uint4* recs;             // deferred big segments {start, count, (set << 1) | type, first chunk}
-  uint4* chunks;           // balanced-phase chunk entries {start, count, set, type}
-  uint32_t recCap, chunkCap;
+  uint4* chunks;           // balanced-phase chunk entries {start, count, alpha, type}
+  uint32_t chunkCap;
   // eager kernel state
   uint2* Q[2];
   int32_t* stamp;  // last level at which a slice set was enqueued
@@ -41,11 +43,14 @@ struct BfsParams {
   Ctrl* ctrl;
   blest_level_trace_t* trace;
   uint32_t traceCap;
-  uint32_t src;  // internal id
+  uint32_t src;      // internal id
+  uint32_t srcOrig;  // original id
   int switching;
   int contraction;
   uint32_t buMask;  // switching == 5: level l runs bottom-up iff bit min(l,31) is set
   float eta, gamma;
+  // switch cost model, picoseconds per unit
+  float cTdEdge, cTdVertex, cTdWord, cBuVertex, cBuScan, cBuWord;
 };
 
 struct MsParams {

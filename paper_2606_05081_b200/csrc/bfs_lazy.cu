@@ -1,21 +1,25 @@
 // bfs_lazy.cu -- single-source BLEST traversal with lazy vertex updates (Alg. 3, :345-455) and the
 // per-level switch to CUDA-core paths (§5.3, Eq. 6, Alg. 4), as ONE persistent cooperative kernel per call
-// (PAPER.md:464, :496).  DESIGN.md "Lazy kernel" explains every deviation from the listing; in short:
+// (PAPER.md:464, :496).  DESIGN.md §5.2 explains every deviation from the listing; in short:
 //
 //   state     one visited bitmap V and three rotating frontier bitmaps (level l reads F[(l-1)%3], marks F[l%3] and
 //             clears F[(l+1)%3]); the paper's V_next XOR V_curr is F[l%3] AND NOT V.
-//   top-down  Stage 1 consumes the list of non-zero frontier WORDS produced by the previous finalisation.  For every
-//             newly active slice set it takes either the slice path -- the pull contraction over the
-//             set's BVSS slices -- or, where the set has few active columns, the CSR edges of
-//             its frontier vertices (the CUDA-core top-down path of north_star (e)).  Short segments are processed in
-//             place, long ones (hub vertices / hub slice sets) are cut into equal chunks and spread over the grid.
-//             Marks are filtered no-return atomic ORs.  Stage 2 is the finalisation sweep
-//             (PAPER.md:399-446): L[u] = l once per discovered vertex, counters, next word list.
+//   top-down  Stage 1 consumes the list of non-zero frontier WORDS produced by the previous finalisation, 32 words per
+//             warp step.  Every newly active slice set takes either the slice path -- the pull
+//             contraction over the set's BVSS quads -- or the CSR edges of its frontier vertices
+//             (the CUDA-core top-down path of north_star (e)).  The segments of the 32 words are flattened with a warp
+//             scan, so that all lanes work whatever the degrees are, and every lane keeps several independent
+//             loads / bitmap probes in flight.  Hub segments are cut into equal chunks and spread over the grid in a
+//             second, balanced phase.  Marks are filtered no-return atomic ORs.  Stage 2 is the
+//             finalisation sweep: level written once per discovered vertex, counters, next word list.
 //   bottom-up Alg. 4 fused with its finalisation: the warp that owns word w of the visited bitmap
-//             decides all 32 bits, so V, F_next, L and the counters are written in the same sweep (one barrier/level).
-//   switch    start of each level: a byte-cost comparison of the two directions from the counters of the previous
+//             decides all 32 bits, so V, F_next, levels and the counters are written in the same sweep (one grid
+//             barrier per level).  The first two neighbours of every vertex are kept inline (`head`), so most
+//             unvisited vertices are resolved by one coalesced 8-byte load and one or two bitmap probes.
+//   switch    start of each level: estimated cost of the two directions from the counters of the previous
 //             finalisation (#unvisited as in Eq. 6, plus degree sums), scaled by eta.
-//   hand-off  levels are written in internal ids (coalesced) and gathered into original ids once at the end (A10).
+//   output    levels_out is pre-filled with -1 ("infinity", reading R1) and the level of a vertex is
+//             written to levels_out[original id] at the moment it is finalised (A10 fused into A6 / Alg. 4).
 #include "bfs_kernels.cuh"
 
 namespace blest {
@@ -23,11 +27,20 @@ namespace blest {
 namespace {
 
 constexpr uint32_t FULL = 0xffffffffu;
+constexpr uint32_t NONE = 0xffffffffu;
+
+constexpr uint32_t BU_LIST = 512;   // per-warp list of unvisited vertices (sparse bottom-up groups)
+constexpr uint32_t BU_BATCH = 256;  // vertices per bottom-up batch: 8 per lane in flight
 
 struct LazyShared {
   unsigned long long acc[6];
+  unsigned long long ctl[4];  // control words of the level, read by one thread and broadcast
   uint32_t wlCnt;
   uint32_t wlBase;
+  uint32_t buFound[WARPS_PER_BLOCK][32];
+  uint32_t buSlotU[WARPS_PER_BLOCK][32];
+  uint32_t buSlotTag[WARPS_PER_BLOCK][32];
+  uint32_t buList[WARPS_PER_BLOCK][BU_LIST];
   uint32_t wl[WL_STAGE];
 };
 
@@ -78,36 +91,110 @@ __device__ __forceinline__ void wl_flush(LazyShared& sh, uint32_t* WLn, unsigned
 __device__ __forceinline__ uint32_t wl_reserve(LazyShared& sh, unsigned int* wlc, uint32_t cnt) {
   const uint32_t pos = atomicAdd(&sh.wlCnt, cnt);
   if (pos + cnt <= WL_STAGE) return pos;
-  for (uint32_t i = pos; i < WL_STAGE; ++i) sh.wl[i] = 0xFFFFFFFFu;
+  for (uint32_t i = pos; i < WL_STAGE; ++i) sh.wl[i] = NONE;
   return 0x80000000u | atomicAdd(wlc, cnt);
 }
 __device__ __forceinline__ void wl_store(LazyShared& sh, uint32_t* WLn, uint32_t slot, uint32_t w) {
   if (slot & 0x80000000u) WLn[slot & 0x7FFFFFFFu] = w;
   else sh.wl[slot] = w;
 }
-
-__device__ __forceinline__ uint32_t valid_mask(const BfsParams& p, uint32_t w) {
-  return (w == p.nwords - 1 && (p.n & 31u)) ? ((1u << (p.n & 31u)) - 1u) : 0xFFFFFFFFu;
+// Warp-level append of the non-zero words among the lanes' (word id, flag) pairs.
+__device__ __forceinline__ void wl_append(LazyShared& sh, uint32_t* WLn, unsigned int* wlc, uint32_t word, bool nonzero,
+                                          uint32_t lane) {
+  const uint32_t nz = __ballot_sync(FULL, nonzero);
+  if (!nz) return;
+  uint32_t base = 0;
+  if (lane == 0) base = wl_reserve(sh, wlc, (uint32_t)__popc(nz));
+  base = __shfl_sync(FULL, base, 0);
+  if (nonzero) wl_store(sh, WLn, base + __popc(nz & ((1u << lane) - 1u)), word);
 }
 
-// Lazy mark: filtered no-return atomic OR into the next frontier.  V does not change during Stage 1,
-// so its read may be served by L1; the frontier word is read at L2.
-struct Marker {
-  const uint32_t* V;
-  uint32_t* Fn;
-  __device__ __forceinline__ void operator()(uint32_t v) const {
-    const uint32_t w = v >> 5, bit = 1u << (v & 31u);
-    if (V[w] & bit) return;
-    if (__ldcg(&Fn[w]) & bit) return;
-    atomicOr(&Fn[w], bit);
-  }
-};
+__device__ __forceinline__ uint32_t valid_mask(const BfsParams& p, uint32_t w) {
+  return (w == p.nwords - 1 && (p.n & 31u)) ? ((1u << (p.n & 31u)) - 1u) : FULL;
+}
 
-// ---- Stage 1 building blocks ------------------------------------------------------------------------------------
-// Pull contraction over quads [a, a+nq) of one slice set with frontier word alpha: per lane a
-// 128-bit row-id load and a 32-bit mask load, four quads in flight.  All 32 lanes take part (the MMA forms need it).
+__device__ __forceinline__ void prefetch_l2(const void* ptr) { asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr)); }
+
+// ---- lazy marks ----------------------------------------------------------------------------------
+// U candidate vertices per lane: filtered no-return atomic ORs into the next frontier.  The probes of the U
+// candidates are issued together (V first: it does not change during Stage 1, so L1 may serve it; then F_next at L2).
+template <int U>
+__device__ __forceinline__ void mark_batch(const uint32_t* V, uint32_t* Fn, const uint32_t (&v)[U], uint32_t valid) {
+  uint32_t vw[U];
+#pragma unroll
+  for (int j = 0; j < U; ++j) vw[j] = ((valid >> j) & 1u) ? V[v[j] >> 5] : FULL;
+  uint32_t need = 0;
+#pragma unroll
+  for (int j = 0; j < U; ++j)
+    if (!((vw[j] >> (v[j] & 31u)) & 1u)) need |= 1u << j;
+  uint32_t fw[U];
+#pragma unroll
+  for (int j = 0; j < U; ++j) fw[j] = ((need >> j) & 1u) ? __ldcg(&Fn[v[j] >> 5]) : FULL;
+#pragma unroll
+  for (int j = 0; j < U; ++j)
+    if (((need >> j) & 1u) && !((fw[j] >> (v[j] & 31u)) & 1u)) atomicOr(&Fn[v[j] >> 5], 1u << (v[j] & 31u));
+}
+
+// Smallest lane whose inclusive prefix exceeds idx (idx < total); all 32 lanes must call.
+__device__ __forceinline__ uint32_t find_owner(uint32_t incl, uint32_t idx) {
+  uint32_t lo = 0;
+#pragma unroll
+  for (int step = 16; step > 0; step >>= 1) {
+    const uint32_t probe = __shfl_sync(FULL, incl, lo + step - 1);
+    if (probe <= idx) lo += step;
+  }
+  return lo;
+}
+
+// CUDA-core top-down: each lane owns one adjacency segment [r0, r0+deg); the warp walks the concatenation.
+__device__ __forceinline__ void expand_edges(const BfsParams& p, uint32_t* Fn, uint32_t r0, uint32_t deg, uint32_t lane) {
+  const uint32_t incl = warp_incl_scan(deg, lane);
+  const uint32_t total = __shfl_sync(FULL, incl, 31);
+  const uint32_t basePtr = r0 - (incl - deg);
+  for (uint32_t base = 0; base < total; base += 128u) {
+    uint32_t v[4], valid = 0;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const uint32_t idx = base + 32u * j + lane;
+      const uint32_t own = find_owner(incl, idx);
+      const uint32_t bp = __shfl_sync(FULL, basePtr, own);
+      v[j] = 0;
+      if (idx < total) {
+        v[j] = __ldcs(p.colidx + (bp + idx));
+        valid |= 1u << j;
+      }
+    }
+    mark_batch<4>(p.V, Fn, v, valid);
+  }
+}
+
+// One contiguous run of edges handled by the whole warp (balanced phase, long adjacency lists).
+__device__ __forceinline__ void warp_edges(const BfsParams& p, uint32_t* Fn, uint32_t e0, uint32_t e1, uint32_t lane) {
+  for (uint32_t base = e0; base < e1; base += 128u) {
+    uint32_t v[4], valid = 0;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const uint32_t idx = base + 32u * j + lane;
+      v[j] = 0;
+      if (idx < e1) {
+        v[j] = __ldcs(p.colidx + idx);
+        valid |= 1u << j;
+      }
+    }
+    mark_batch<4>(p.V, Fn, v, valid);
+  }
+}
+
+__device__ __forceinline__ void mark_quad(const BfsParams& p, uint32_t* Fn, const uint4& r, uint32_t hits) {
+  const uint32_t v[4] = {r.x, r.y, r.z, r.w};
+  mark_batch<4>(p.V, Fn, v, hits);
+}
+
+// Pull contraction over quads [a, a+nq) of ONE slice set with frontier word alpha: per lane a
+// 128-bit row-id load and a 32-bit mask load, four quads in flight.  alpha is warp-uniform, all 32 lanes take part
+// (the MMA forms of the contraction need both).
 template <int CONTR>
-__device__ __forceinline__ void warp_slices(const BfsParams& p, const Marker& mk, uint32_t a, uint32_t nq, uint32_t alpha,
+__device__ __forceinline__ void warp_slices(const BfsParams& p, uint32_t* Fn, uint32_t a, uint32_t nq, uint32_t alpha,
                                             uint32_t lane) {
   for (uint32_t base = 0; base < nq; base += 128u) {
     uint4 r[4];
@@ -126,130 +213,224 @@ __device__ __forceinline__ void warp_slices(const BfsParams& p, const Marker& mk
     for (int k = 0; k < 4; ++k) {
       if (base + 32u * k < nq) {  // warp-uniform
         const uint32_t hits = contract<CONTR>(m[k], alpha, lane);
-        if (hits & 1u) mk(r[k].x);
-        if (hits & 2u) mk(r[k].y);
-        if (hits & 4u) mk(r[k].z);
-        if (hits & 8u) mk(r[k].w);
+        mark_quad(p, Fn, r[k], hits);
       }
     }
   }
 }
 
-// CUDA-core top-down: every edge out of a frontier vertex is a mark candidate.
-__device__ __forceinline__ void warp_edges(const BfsParams& p, const Marker& mk, uint32_t e0, uint32_t e1, uint32_t lane) {
-  for (uint32_t base = e0; base < e1; base += 128u) {
-    uint32_t v[4];
-    bool ok[4];
+// Slice path, flattened: each lane owns the quads [a, a+nq) of one slice set with its own frontier word alpha; the
+// warp walks the concatenation, two quads per lane in flight (ALU contraction: it needs no warp-uniform alpha).
+__device__ __forceinline__ void expand_slices(const BfsParams& p, uint32_t* Fn, uint32_t a, uint32_t nq, uint32_t alpha,
+                                              uint32_t lane) {
+  const uint32_t incl = warp_incl_scan(nq, lane);
+  const uint32_t total = __shfl_sync(FULL, incl, 31);
+  const uint32_t basePtr = a - (incl - nq);
+  for (uint32_t base = 0; base < total; base += 64u) {
+    uint4 r[2];
+    uint32_t m[2], al[2];
+    bool ok[2];
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const uint32_t idx = base + 32u * k + lane;
-      ok[k] = idx < e1;
-      v[k] = ok[k] ? __ldcs(p.colidx + idx) : 0u;
+    for (int j = 0; j < 2; ++j) {
+      const uint32_t idx = base + 32u * j + lane;
+      const uint32_t own = find_owner(incl, idx);
+      const uint32_t bp = __shfl_sync(FULL, basePtr, own);
+      al[j] = __shfl_sync(FULL, alpha, own);
+      ok[j] = idx < total;
+      r[j] = make_uint4(0, 0, 0, 0);
+      m[j] = 0;
+      if (ok[j]) {
+        r[j] = __ldcs(p.rowIds + (bp + idx));
+        m[j] = __ldcs(p.masks + (bp + idx));
+      }
     }
 #pragma unroll
-    for (int k = 0; k < 4; ++k)
-      if (ok[k]) mk(v[k]);
+    for (int j = 0; j < 2; ++j)
+      if (__any_sync(FULL, ok[j])) mark_quad(p, Fn, r[j], contract_alu(m[j], al[j]));
   }
 }
 
-__device__ __forceinline__ void push_record(const BfsParams& p, Ctrl* ctrl, uint32_t ci, uint32_t type, uint32_t start,
-                                            uint32_t count, uint32_t s) {
+// A hub segment (long adjacency list / big slice set) is cut into equal chunks by the warp that found it; the chunks
+// are consumed by the whole grid in the balanced phase.
+__device__ __forceinline__ void emit_chunks(const BfsParams& p, Ctrl* ctrl, uint32_t ci, uint32_t type, uint32_t start,
+                                            uint32_t count, uint32_t alpha, uint32_t lane) {
   const uint32_t per = type ? CHUNK_EDGES : CHUNK_QUADS;
   const uint32_t nent = (count + per - 1) / per;
-  const uint32_t idx = atomicAdd(&ctrl->nBig[ci], 1u);
-  const uint32_t pos = atomicAdd(&ctrl->qc[ci], nent);
-  if (idx < p.recCap && (uint64_t)pos + nent <= p.chunkCap) p.recs[idx] = make_uint4(start, count, (s << 1) | type, pos);
-  else atomicOr(&ctrl->error, 1u);
+  uint32_t pos = 0;
+  if (lane == 0) {
+    pos = atomicAdd(&ctrl->qc[ci], nent);
+    atomicAdd(&ctrl->nBig[ci], 1u);
+  }
+  pos = __shfl_sync(FULL, pos, 0);
+  if ((uint64_t)pos + nent > p.chunkCap) {
+    if (lane == 0) atomicOr(&ctrl->error, 1u);
+    return;
+  }
+  for (uint32_t i = lane; i < nent; i += 32) p.chunks[pos + i] = make_uint4(start + i * per, min(per, count - i * per), alpha, type);
 }
 
-// Stage 1, top-down, phase A: one warp per non-zero frontier word.
+// Stage 1, top-down, phase A: 32 non-zero frontier words per warp step (lane = word).
 template <int CONTR>
 __device__ __forceinline__ void td_phase_a(const BfsParams& p, LazyShared& sh, const uint32_t* WLc, uint32_t wlCount,
                                            const uint32_t* Fp, uint32_t* Fn, Ctrl* ctrl, uint32_t ci) {
   const uint32_t lane = threadIdx.x & 31;
   const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
-  const Marker mk{p.V, Fn};
-  const bool slicesAllowed = (p.switching != 3);
-  const bool edgesAllowed = (p.switching != 1 && p.switching != 4);
+  const int sw = p.switching;
+  // words per warp step: 32 when the list is long; fewer when it is short, so that a small frontier still spreads
+  // over the grid (one word per warp below nwarps words)
+  const uint32_t W = min(32u, max(1u, (wlCount + nwarps - 1) / nwarps));
   Counters c;
-  for (uint32_t i = gwarp; i < wlCount; i += nwarps) {
-    const uint32_t t = __ldcg(&WLc[i]);
-    if (t == 0xFFFFFFFFu) continue;  // staging sentinel (wl_reserve)
-    const uint32_t fw = Fp[t];
-    const uint32_t u = t * 32u + lane;
-    const bool mine = (fw >> lane) & 1u;
-    uint32_t r0 = 0, deg = 0;
-    if (mine) {
-      r0 = __ldg(&p.rowptr[u]);
-      deg = __ldg(&p.rowptr[u + 1]) - r0;
+  for (uint32_t i0 = gwarp * W; i0 < wlCount; i0 += nwarps * W) {
+    const uint32_t i = i0 + lane;
+    uint32_t t = NONE, fw = 0, thr = 0x9999u;
+    if (lane < W && i < wlCount) t = __ldcg(&WLc[i]);
+    if (t != NONE) {  // NONE: staging sentinel (wl_reserve)
+      fw = Fp[t];
+      if (sw == 0 || sw == 5) thr = __ldg(&p.popThr[t]);
     }
-    // the 8 lanes of group k = lane >> 3 stand for the 8 columns of slice set s = 4t + k
-    uint32_t ds = deg;
-    ds += __shfl_xor_sync(FULL, ds, 1);
-    ds += __shfl_xor_sync(FULL, ds, 2);
-    ds += __shfl_xor_sync(FULL, ds, 4);
-    const uint32_t k = lane >> 3, s = t * 4u + k, byte = (fw >> (8u * k)) & 0xFFu;
-    uint32_t a = 0, nq = 0;
-    if (byte && slicesAllowed) {
-      a = __ldg(&p.setPtr[s]);
-      nq = __ldg(&p.setPtr[s + 1]) - a;
+    // which of the word's four slice sets take the slice path: forced, or by the build-time threshold on the number
+    // of frontier columns
+    uint32_t smask = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const uint32_t byte = (fw >> (8 * k)) & 0xFFu;
+      bool use = false;
+      if (byte) {
+        if (sw == 1 || sw == 4) use = true;
+        else if (sw == 3) use = false;
+        else use = (uint32_t)__popc(byte) >= ((thr >> (4 * k)) & 15u);
+      }
+      if (use) smask |= 1u << k;
     }
-    // slice path unless the set's active columns own fewer bytes as CSR edges (4 B per edge + row pointers) than
-    // the whole set does as slices (20 B per quad); gamma scales the comparison (measured)
-    bool useSlice = byte && nq && slicesAllowed;
-    if (useSlice && edgesAllowed && 4.0f * (float)ds + 16.0f * (float)__popc(byte) < p.gamma * 20.0f * (float)nq) useSlice = false;
-    const bool edgeMine = mine && !useSlice && deg > 0;
-    if (edgeMine) c.qbytes += 4ull * deg;
-    if (useSlice && (lane & 7u) == 0) c.qbytes += 20ull * nq;
-    // (1) short adjacency lists: the owning lane scans them itself
-    if (edgeMine && deg <= TINY_DEG)
-      for (uint32_t e = r0; e < r0 + deg; ++e) mk(__ldcs(p.colidx + e));
-    // (2) medium lists: the warp scans them together; long ones are deferred
-    uint32_t pend = __ballot_sync(FULL, edgeMine && deg > TINY_DEG);
-    while (pend) {
-      const int srcLane = __ffs(pend) - 1;
-      pend &= pend - 1;
-      const uint32_t R0 = __shfl_sync(FULL, r0, srcLane), D = __shfl_sync(FULL, deg, srcLane);
-      if (D <= BIG_EDGES) warp_edges(p, mk, R0, R0 + D, lane);
-      else if (lane == 0) push_record(p, ctrl, ci, 1u, R0, D, 0u);
+    uint32_t ebits = fw;
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if ((smask >> k) & 1u) ebits &= ~(0xFFu << (8 * k));
+    // ---- slice path
+    if (__any_sync(FULL, smask != 0)) {
+      uint32_t a[4], nq[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        a[k] = nq[k] = 0;
+        if ((smask >> k) & 1u) {
+          const uint32_t s = t * 4u + k;
+          a[k] = __ldg(&p.setPtr[s]);
+          nq[k] = __ldg(&p.setPtr[s + 1]) - a[k];
+          c.qbytes += 20ull * nq[k] + 8ull;
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        if (!__any_sync(FULL, nq[k] != 0)) continue;
+        const uint32_t alpha = (fw >> (8 * k)) & 0xFFu;
+        // hub sets -> balanced phase; with an MMA contraction every set is walked by the whole warp (uniform alpha)
+        uint32_t big = __ballot_sync(FULL, nq[k] > (CONTR == 1 ? BIG_QUADS : 0u));
+        while (big) {
+          const int src = __ffs(big) - 1;
+          big &= big - 1;
+          const uint32_t A = __shfl_sync(FULL, a[k], src), NQ = __shfl_sync(FULL, nq[k], src), AL = __shfl_sync(FULL, alpha, src);
+          if (NQ > BIG_QUADS) emit_chunks(p, ctrl, ci, 0u, A, NQ, AL, lane);
+          else warp_slices<CONTR>(p, Fn, A, NQ, AL, lane);
+        }
+        if (CONTR == 1) expand_slices(p, Fn, a[k], nq[k] > BIG_QUADS ? 0u : nq[k], alpha, lane);
+      }
     }
-    // (3) slice sets: contraction over the set's quads; hub sets are deferred
-    uint32_t pendS = __ballot_sync(FULL, useSlice && (lane & 7u) == 0);
-    while (pendS) {
-      const int srcLane = __ffs(pendS) - 1;
-      pendS &= pendS - 1;
-      const uint32_t A = __shfl_sync(FULL, a, srcLane), NQ = __shfl_sync(FULL, nq, srcLane);
-      const uint32_t AL = __shfl_sync(FULL, byte, srcLane), S = __shfl_sync(FULL, s, srcLane);
-      if (NQ <= BIG_QUADS) warp_slices<CONTR>(p, mk, A, NQ, AL, lane);
-      else if (lane == 0) push_record(p, ctrl, ci, 0u, A, NQ, S);
+    // ---- CUDA-core edge path: up to four frontier vertices per lane and round
+    while (__any_sync(FULL, ebits != 0)) {
+      uint32_t r0[4], deg[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        r0[q] = deg[q] = 0;
+        if (ebits) {
+          const uint32_t u = t * 32u + (uint32_t)(__ffs(ebits) - 1);
+          ebits &= ebits - 1;
+          r0[q] = __ldg(&p.rowptr[u]);
+          deg[q] = __ldg(&p.rowptr[u + 1]) - r0[q];
+          c.qbytes += 8ull;
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        if (!__any_sync(FULL, deg[q] != 0)) continue;
+        c.qbytes += 4ull * deg[q];
+        uint32_t big = __ballot_sync(FULL, deg[q] > BIG_EDGES);
+        while (big) {
+          const int src = __ffs(big) - 1;
+          big &= big - 1;
+          emit_chunks(p, ctrl, ci, 1u, __shfl_sync(FULL, r0[q], src), __shfl_sync(FULL, deg[q], src), 0u, lane);
+        }
+        expand_edges(p, Fn, r0[q], deg[q] > BIG_EDGES ? 0u : deg[q], lane);
+      }
     }
   }
   block_accumulate(sh, c, ctrl, ci);
 }
 
-// Phase B1: one warp per deferred segment writes its chunk entries (32 per step).
-__device__ __forceinline__ void td_phase_b1(const BfsParams& p, uint32_t nBig) {
+// Phase B: one warp per chunk, round-robin: every warp gets the same share of the hubs' bytes.
+template <int CONTR>
+__device__ __forceinline__ void td_phase_b(const BfsParams& p, uint32_t nChunks, uint32_t* Fn) {
   const uint32_t lane = threadIdx.x & 31;
   const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
-  for (uint32_t r = gwarp; r < nBig; r += nwarps) {
-    const uint4 rec = p.recs[r];
-    const uint32_t type = rec.z & 1u, s = rec.z >> 1, per = type ? CHUNK_EDGES : CHUNK_QUADS;
-    const uint32_t nent = (rec.y + per - 1) / per;
-    for (uint32_t i = lane; i < nent; i += 32) p.chunks[rec.w + i] = make_uint4(rec.x + i * per, min(per, rec.y - i * per), s, type);
+  for (uint32_t i = gwarp; i < nChunks; i += nwarps) {
+    const uint4 e = __ldcg(&p.chunks[i]);
+    if (e.w) warp_edges(p, Fn, e.x, e.x + e.y, lane);
+    else warp_slices<CONTR>(p, Fn, e.x, e.y, e.z, lane);
   }
 }
 
-// Phase B2: one warp per chunk, round-robin: every warp gets the same share of the hubs' bytes.
-template <int CONTR>
-__device__ __forceinline__ void td_phase_b2(const BfsParams& p, uint32_t nChunks, const uint32_t* Fp, uint32_t* Fn) {
-  const uint32_t lane = threadIdx.x & 31;
-  const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
-  const Marker mk{p.V, Fn};
-  const uint8_t* Fbytes = reinterpret_cast<const uint8_t*>(Fp);
-  for (uint32_t i = gwarp; i < nChunks; i += nwarps) {
-    const uint4 e = __ldcg(&p.chunks[i]);
-    if (e.w) warp_edges(p, mk, e.x, e.x + e.y, lane);
-    else warp_slices<CONTR>(p, mk, e.x, e.y, Fbytes[e.z], lane);
+// levels_out[original id of u] = level, for the set bits of up to eight words at a time (lane = bit: coalesced
+// iperm / degree loads); also the degree sum of the new frontier for the switch.
+__device__ __forceinline__ void write_levels_dense(const BfsParams& p, uint32_t wordBase, uint32_t fm, uint32_t sel,
+                                                   int32_t level, uint32_t lane, Counters& c) {
+  while (sel) {
+    uint32_t u[8], on = 0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      u[q] = 0;
+      if (sel) {
+        const int src = __ffs(sel) - 1;
+        sel &= sel - 1;
+        const uint32_t f = __shfl_sync(FULL, fm, src);
+        on |= ((f >> lane) & 1u) << q;
+        u[q] = (wordBase + src) * 32u + lane;
+      }
+    }
+    uint32_t o[8], dg[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) o[q] = ((on >> q) & 1u) ? (p.iperm ? __ldg(&p.iperm[u[q]]) : u[q]) : 0u;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) dg[q] = ((on >> q) & 1u) ? __ldg(&p.deg[u[q]]) : 0u;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) c.mf += dg[q];
+#pragma unroll
+    for (int q = 0; q < 8; ++q)
+      if ((on >> q) & 1u) p.out[o[q]] = level;
+  }
+}
+// Same for a lane's own sparse word (a few bits): four vertices in flight.
+__device__ __forceinline__ void write_levels_sparse(const BfsParams& p, uint32_t t, uint32_t bits, int32_t level, Counters& c) {
+  while (bits) {
+    uint32_t u[4], o[4];
+    bool on[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      on[q] = bits != 0;
+      u[q] = 0;
+      if (bits) {
+        u[q] = t * 32u + (uint32_t)(__ffs(bits) - 1);
+        bits &= bits - 1;
+      }
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) o[q] = on[q] ? (p.iperm ? __ldg(&p.iperm[u[q]]) : u[q]) : 0u;
+    uint32_t dg[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) dg[q] = on[q] ? __ldg(&p.deg[u[q]]) : 0u;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) c.mf += dg[q];
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+      if (on[q]) p.out[o[q]] = level;
   }
 }
 
@@ -271,148 +452,329 @@ __device__ __forceinline__ void td_finalize(const BfsParams& p, LazyShared& sh, 
       c.unv += __popc(~(v | fm) & valid_mask(p, t));
       c.nnew += __popc(fm);
     }
-    uint32_t nz = __ballot_sync(FULL, fm != 0);
-    if (nz) {
-      // next level's work list (PAPER.md:420-440 enqueues the VSSs of every newly active slice set; here the non-zero
-      // frontier word is the unit, expanded at consumption time)
-      uint32_t base = 0;
-      if (lane == 0) base = wl_reserve(sh, &ctrl->wlc[ci], (uint32_t)__popc(nz));
-      base = __shfl_sync(FULL, base, 0);
-      if (fm) wl_store(sh, WLn, base + __popc(nz & ((1u << lane) - 1u)), t);
-      // L[u] = level once per discovered vertex, 32 consecutive vertices per step; degree sum for the switch
-      while (nz) {
-        const int srcLane = __ffs(nz) - 1;
-        nz &= nz - 1;
-        const uint32_t f = __shfl_sync(FULL, fm, srcLane);
-        if ((f >> lane) & 1u) {
-          const uint32_t u = (wb + srcLane) * 32u + lane;
-          p.L[u] = (int32_t)level;
-          c.mf += __ldg(&p.rowptr[u + 1]) - __ldg(&p.rowptr[u]);
-        }
-      }
-    }
+    if (!__any_sync(FULL, fm != 0)) continue;
+    // next level's work list (PAPER.md:420-440 enqueues the VSSs of every newly active slice set; here the non-zero
+    // frontier word is the unit, expanded at consumption time)
+    wl_append(sh, WLn, &ctrl->wlc[ci], t, fm != 0, lane);
+    // level once per discovered vertex: dense words by the warp (lane = bit), sparse ones by their lane
+    const bool dense = __popc(fm) > 6;
+    write_levels_dense(p, wb, fm, __ballot_sync(FULL, dense), (int32_t)level, lane, c);
+    if (!dense) write_levels_sparse(p, t, fm, (int32_t)level, c);
   }
   wl_flush(sh, WLn, &ctrl->wlc[ci]);
   block_accumulate(sh, c, ctrl, ci);
 }
 
-// Bottom-up level (Alg. 4, :466-494) fused with its finalisation.  Four words per warp step: the loads of
-// the visited words, row pointers, first neighbours and their frontier bits are independent across the four.
-__device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uint32_t level, const uint32_t* Fp, uint32_t* Fn,
-                                         uint32_t* Fs, uint32_t* WLn, Ctrl* ctrl, uint32_t ci) {
-  constexpr int K = 4;
+// ---- bottom-up (Alg. 4, :466-494) fused with its finalisation ---------------------------------------------
+// Resolve up to 8 unvisited vertices per lane (u[k], NONE = no vertex): does u have a neighbour in the frontier Fp?
+// Inline heads first (one coalesced 8-byte load: first two neighbours), then -- for the few vertices with more than two
+// neighbours and neither of the first two in the frontier -- the CSR scan of PAPER.md:479-487 from the third neighbour
+// on, compacted over the warp (one such vertex per lane and round, four neighbours in flight).  Returns the lane's
+// 8-bit found mask.  All 32 lanes must call.
+constexpr uint32_t CSR_STAGE = 0x80000000u;  // list entry flag: heads already checked, continue with the CSR scan
+
+template <bool DEFER>
+__device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_t* Fp, uint32_t* fshare, uint32_t* slotU,
+                                               uint32_t* slotTag, uint32_t lane, const uint32_t (&u)[8], Counters& c,
+                                               uint32_t* list, uint32_t& listCount) {
+  constexpr int K = 8;
   constexpr uint32_t SERIAL_CAP = 64;
-  const uint32_t lane = threadIdx.x & 31;
-  const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
-  const uint32_t nSW = p.nSweepWords;
-  Counters c;
-  auto in_frontier = [&](uint32_t v) -> bool { return (Fp[v >> 5] >> (v & 31u)) & 1u; };
-  for (uint32_t w0 = gwarp; w0 < nSW; w0 += nwarps * K) {
-    uint32_t cur[K], b[K], e[K];
-    bool act[K], found[K];
+  uint2 h[K];
+  uint32_t act = 0, staged = 0;
 #pragma unroll
-    for (int k = 0; k < K; ++k) {
-      const uint32_t w = w0 + k * nwarps;
-      cur[k] = (w < nSW) ? __ldcg(&p.V[w]) : 0xFFFFFFFFu;
-    }
-#pragma unroll
-    for (int k = 0; k < K; ++k) {
-      const uint32_t w = w0 + k * nwarps;
-      const uint32_t unv = (w < nSW) ? (~cur[k] & valid_mask(p, w)) : 0u;  // padding bits read as visited (R11)
-      act[k] = (unv >> lane) & 1u;
-      b[k] = e[k] = 0;
-      if (act[k]) {
-        const uint32_t u = w * 32u + lane;
-        b[k] = __ldg(&p.rowptr[u]);
-        e[k] = __ldg(&p.rowptr[u + 1]);
+  for (int k = 0; k < K; ++k) {
+    h[k] = make_uint2(NONE, NONE);
+    if (u[k] != NONE) {
+      if (!DEFER && (u[k] & CSR_STAGE)) staged |= 1u << k;
+      else {
+        h[k] = __ldcs(&p.head[u[k]]);
+        act |= 1u << k;
       }
-    }
-    uint32_t v0[K];
-#pragma unroll
-    for (int k = 0; k < K; ++k) v0[k] = (b[k] < e[k]) ? __ldg(&p.colidx[b[k]]) : 0xFFFFFFFFu;
-#pragma unroll
-    for (int k = 0; k < K; ++k) {
-      found[k] = false;
-      if (v0[k] != 0xFFFFFFFFu) {
-        found[k] = in_frontier(v0[k]);
-        ++c.scanned;
-      }
-    }
-#pragma unroll
-    for (int k = 0; k < K; ++k) {
-      // remaining neighbours: the owning lane scans a bounded number, the warp finishes long lists together
-      uint32_t ptr = b[k] + 1;
-      bool more = false;
-      if (b[k] < e[k] && !found[k]) {
-        const uint32_t stop = min(e[k], ptr + SERIAL_CAP);
-        for (; ptr < stop; ++ptr) {
-          ++c.scanned;
-          if (in_frontier(__ldg(&p.colidx[ptr]))) { found[k] = true; break; }
-        }
-        more = !found[k] && ptr < e[k];
-      }
-      uint32_t pend = __ballot_sync(FULL, more);
-      while (pend) {
-        const int srcLane = __ffs(pend) - 1;
-        pend &= pend - 1;
-        const uint32_t B = __shfl_sync(FULL, ptr, srcLane), E = __shfl_sync(FULL, e[k], srcLane);
-        bool f = false;
-        for (uint32_t base = B; base < E; base += 32u) {
-          const uint32_t idx = base + lane;
-          const bool h = idx < E && in_frontier(__ldg(&p.colidx[idx]));
-          c.scanned += idx < E;
-          if (__ballot_sync(FULL, h)) { f = true; break; }
-        }
-        if ((int)lane == srcLane) found[k] = f;
-      }
-    }
-    uint32_t wl[K], wlN = 0;
-#pragma unroll
-    for (int k = 0; k < K; ++k) {
-      const uint32_t w = w0 + k * nwarps;
-      const uint32_t fm = __ballot_sync(FULL, found[k]);
-      if (w < nSW) {
-        if (found[k]) {
-          p.L[w * 32u + lane] = (int32_t)level;  // coalesced: lane = bit index
-          c.mf += e[k] - b[k];
-        }
-        if (lane == 0) {
-          if (fm) p.V[w] = cur[k] | fm;  // this warp owns word w: no atomic (PAPER.md:483 needs one per lane)
-          Fn[w] = fm;
-          Fs[w] = 0;
-          c.nnew += __popc(fm);
-          c.unv += __popc(~(cur[k] | fm) & valid_mask(p, w));
-          if (fm) wl[wlN++] = w;
-        }
-      }
-    }
-    if (lane == 0 && wlN) {
-      const uint32_t base = wl_reserve(sh, &ctrl->wlc[ci], wlN);
-      for (uint32_t i = 0; i < wlN; ++i) wl_store(sh, WLn, base + i, wl[i]);
     }
   }
+  c.qbytes += 8ull * __popc(act);
+  uint32_t found = 0;
+  {
+    uint32_t f[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) f[k] = (h[k].x != NONE) ? Fp[h[k].x >> 5] : 0u;
+#pragma unroll
+    for (int k = 0; k < K; ++k)
+      if (h[k].x != NONE) {
+        ++c.scanned;
+        if ((f[k] >> (h[k].x & 31u)) & 1u) found |= 1u << k;
+      }
+  }
+  uint32_t need = 0;
+#pragma unroll
+  for (int k = 0; k < K; ++k)
+    if (h[k].y != NONE && !((found >> k) & 1u)) need |= 1u << k;
+  if (__any_sync(FULL, need != 0)) {
+    uint32_t f[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) f[k] = ((need >> k) & 1u) ? Fp[(h[k].y & 0x7FFFFFFFu) >> 5] : 0u;
+#pragma unroll
+    for (int k = 0; k < K; ++k)
+      if ((need >> k) & 1u) {
+        ++c.scanned;
+        if ((f[k] >> (h[k].y & 31u)) & 1u) found |= 1u << k;
+      }
+  }
+  uint32_t more = staged;
+#pragma unroll
+  for (int k = 0; k < K; ++k)
+    if (((need >> k) & 1u) && !((found >> k) & 1u) && (h[k].y >> 31)) more |= 1u << k;
+  if (!__any_sync(FULL, more != 0)) return found;
+
+  uint32_t pos[K], total = 0;  // position of the lane's k-th vertex in the warp-wide list of such vertices
+  const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll
+  for (int k = 0; k < K; ++k) {
+    const uint32_t bal = __ballot_sync(FULL, (more >> k) & 1u);
+    pos[k] = total + __popc(bal & lt);
+    total += __popc(bal);
+  }
+  if (DEFER) {  // in-place (dense) mode: these vertices join the warp's list and are resolved later, 256 at a time
+#pragma unroll
+    for (int k = 0; k < K; ++k)
+      if ((more >> k) & 1u) {
+        list[listCount + pos[k]] = u[k] | CSR_STAGE;
+        prefetch_l2(&p.rowptr[u[k]]);
+      }
+    listCount += total;
+    __syncwarp();
+    return found;
+  }
+  fshare[lane] = 0;
+  for (uint32_t base = 0; base < total; base += 32u) {
+    __syncwarp();
+#pragma unroll
+    for (int k = 0; k < K; ++k)
+      if (((more >> k) & 1u) && pos[k] >= base && pos[k] < base + 32u) {
+        slotU[pos[k] - base] = u[k];
+        slotTag[pos[k] - base] = (uint32_t)k | (lane << 3);
+      }
+    __syncwarp();
+    const bool mine = base + lane < total;
+    uint32_t ptr = 0, e = 0, tag = 0;
+    if (mine) {
+      const uint32_t uu = slotU[lane] & ~CSR_STAGE;
+      tag = slotTag[lane];
+      ptr = __ldg(&p.rowptr[uu]) + 2u;
+      e = __ldg(&p.rowptr[uu + 1]);
+      c.qbytes += 8ull;
+    }
+    bool f = false;
+    const uint32_t stop = min(e, ptr + SERIAL_CAP);
+    while (!f && ptr < stop) {  // four neighbours per step
+      uint32_t v[4], fwd[4];
+      const uint32_t cnt = min(4u, stop - ptr);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) v[j] = (uint32_t)j < cnt ? __ldg(&p.colidx[ptr + j]) : 0u;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) fwd[j] = (uint32_t)j < cnt ? Fp[v[j] >> 5] : 0u;
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+        if ((uint32_t)j < cnt && ((fwd[j] >> (v[j] & 31u)) & 1u)) f = true;
+      c.scanned += cnt;
+      c.qbytes += 4ull * cnt;
+      ptr += cnt;
+    }
+    // long lists are finished by the whole warp
+    uint32_t pend = __ballot_sync(FULL, mine && !f && ptr < e);
+    while (pend) {
+      const int src = __ffs(pend) - 1;
+      pend &= pend - 1;
+      const uint32_t B = __shfl_sync(FULL, ptr, src), E = __shfl_sync(FULL, e, src);
+      bool ff = false;
+      for (uint32_t b2 = B; b2 < E; b2 += 32u) {
+        const uint32_t idx = b2 + lane;
+        bool hit = false;
+        if (idx < E) {
+          const uint32_t v = __ldg(&p.colidx[idx]);
+          hit = (Fp[v >> 5] >> (v & 31u)) & 1u;
+          ++c.scanned;
+          c.qbytes += 4ull;
+        }
+        if (__ballot_sync(FULL, hit)) { ff = true; break; }
+      }
+      if ((int)lane == src) f = ff;
+    }
+    if (mine && f) atomicOr(&fshare[tag >> 3], 1u << (tag & 7u));
+  }
+  __syncwarp();
+  found |= fshare[lane];
+  __syncwarp();
+  return found;
+}
+
+// One bottom-up level.  A warp step covers a GROUP of G words of the visited bitmap (lane = word; G = 8 on levels with
+// many unvisited vertices so that the groups balance over the grid, 32 otherwise).  Dense groups are resolved in
+// place, 8 words at a time with lane = bit, and the warp that owns the words writes V / F_next / levels without
+// atomics; what the inline heads cannot decide goes to the warp's list.  The unvisited vertices of sparse groups go to
+// the list directly.  The list is resolved 256 vertices at a time whatever words they come from (atomics on
+// V / F_next: they are few), so a level with few unvisited vertices costs one sweep of V plus work proportional to
+// their number.
+__device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uint32_t level, const uint32_t* Fp, uint32_t* Fn,
+                                         uint32_t* Fs, uint32_t* WLn, Ctrl* ctrl, uint32_t ci, unsigned long long nu) {
+  const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + warp, nwarps = gridDim.x * WARPS_PER_BLOCK;
+  const uint32_t nSW = p.nSweepWords;
+  const uint32_t G = (nu * 8ull > (unsigned long long)nSW * 32ull) ? 8u : 32u;  // > 1/8 of the sweep range unvisited
+  const uint32_t nGroups = (nSW + G - 1u) / G;
+  uint32_t* fshare = sh.buFound[warp];
+  uint32_t* slotU = sh.buSlotU[warp];
+  uint32_t* slotTag = sh.buSlotTag[warp];
+  uint32_t* list = sh.buList[warp];
+  uint32_t listCount = 0;
+  bool batchRan = false;  // a list batch ran since the current group started
+  Counters c;
+
+  // resolve the last `cnt` (<= 256) vertices of the list
+  auto run_batch = [&](uint32_t cnt) {
+    const uint32_t start = listCount - cnt;
+    uint32_t u[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) u[k] = (32u * k + lane < cnt) ? list[start + 32u * k + lane] : NONE;
+    __syncwarp();
+    listCount = start;
+    const uint32_t found = bu_resolve<false>(p, Fp, fshare, slotU, slotTag, lane, u, c, list, listCount);
+    uint32_t o[8], dg[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) o[k] = ((found >> k) & 1u) ? (p.iperm ? __ldg(&p.iperm[u[k] & ~CSR_STAGE]) : (u[k] & ~CSR_STAGE)) : 0u;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) dg[k] = ((found >> k) & 1u) ? __ldg(&p.deg[u[k] & ~CSR_STAGE]) : 0u;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) c.mf += dg[k];
+    batchRan = true;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      bool newWord = false;
+      const uint32_t uu = u[k] & ~CSR_STAGE;
+      if ((found >> k) & 1u) {
+        p.out[o[k]] = (int32_t)level;
+        const uint32_t bit = 1u << (uu & 31u);
+        atomicOr(&p.V[uu >> 5], bit);
+        newWord = atomicOr(&Fn[uu >> 5], bit) == 0u;  // first bit of the word in this level: the word joins the list
+      }
+      wl_append(sh, WLn, &ctrl->wlc[ci], uu >> 5, newWord, lane);
+    }
+    c.nnew += __popc(found);
+    c.unv -= __popc(found);
+  };
+
+  for (uint32_t g = gwarp; g < nGroups; g += nwarps) {
+    const uint32_t gw = g * G, myw = gw + lane;
+    const bool wlane = lane < G && myw < nSW;
+    uint32_t curw = FULL;
+    if (wlane) curw = __ldcg(&p.V[myw]);
+    const uint32_t unvw = wlane ? (~curw & valid_mask(p, myw)) : 0u;  // padding bits read as visited (R11)
+    if (wlane) Fs[myw] = 0;  // the frontier of two levels ago becomes the clean F_next of the next level
+    const uint32_t cnt = __popc(unvw);
+    const uint32_t incl = warp_incl_scan(cnt, lane);
+    const uint32_t total = __shfl_sync(FULL, incl, 31);
+    if (total == 0) continue;
+    c.unv += cnt;
+    batchRan = false;
+    if (total > 8u * G) {
+      // ---- dense group (> 1/4 unvisited): in place, 8 words at a time (lane = bit)
+      uint32_t fmw = 0;  // new frontier bits of word myw
+      const uint32_t nzWords = __ballot_sync(FULL, unvw != 0);
+#pragma unroll 1
+      for (uint32_t sub = 0; sub < G / 8u; ++sub) {
+        if (!((nzWords >> (8u * sub)) & 0xFFu)) continue;
+        if (listCount >= BU_BATCH) run_batch(BU_BATCH);  // room for up to 256 deferred vertices
+        uint32_t u[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const uint32_t wbits = __shfl_sync(FULL, unvw, 8u * sub + k);
+          u[k] = ((wbits >> lane) & 1u) ? (gw + 8u * sub + k) * 32u + lane : NONE;
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k)  // the write-back reads these: start the lines towards L2 now
+          if (u[k] != NONE) {
+            if (p.iperm) prefetch_l2(&p.iperm[u[k]]);
+            prefetch_l2(&p.deg[u[k]]);
+          }
+        if (sub + 1 < G / 8u) {  // and the heads of the next 8 words
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {
+            const uint32_t wbits = __shfl_sync(FULL, unvw, (8u * sub + 8u + k) & 31u);
+            if ((wbits >> lane) & 1u) prefetch_l2(&p.head[(size_t)(gw + 8u * sub + 8u + k) * 32u + lane]);
+          }
+        }
+        const uint32_t found = bu_resolve<true>(p, Fp, fshare, slotU, slotTag, lane, u, c, list, listCount);
+        uint32_t o[8], dg[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) o[k] = ((found >> k) & 1u) ? (p.iperm ? __ldg(&p.iperm[u[k]]) : u[k]) : 0u;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) dg[k] = ((found >> k) & 1u) ? __ldg(&p.deg[u[k]]) : 0u;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) c.mf += dg[k];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          if ((found >> k) & 1u) p.out[o[k]] = (int32_t)level;  // lane = bit: coalesced when there is no reordering
+          const uint32_t fmk = __ballot_sync(FULL, (found >> k) & 1u);
+          if (lane == 8u * sub + k) fmw = fmk;
+        }
+      }
+      // one atomic per word instead of one per lane; atomic because vertices of this word that were
+      // deferred to the list may already have been resolved by run_batch
+      bool newWord = false;
+      if (fmw) {
+        if (batchRan) {  // (warp-uniform) deferred vertices of this group may already have set bits in these words
+          atomicOr(&p.V[myw], fmw);
+          newWord = atomicOr(&Fn[myw], fmw) == 0u;
+        } else {
+          p.V[myw] = curw | fmw;
+          Fn[myw] = fmw;
+          newWord = true;
+        }
+      }
+      __syncwarp();  // the plain stores precede this warp's later atomics on the same words (deferred vertices)
+      c.nnew += __popc(fmw);
+      c.unv -= __popc(fmw);
+      wl_append(sh, WLn, &ctrl->wlc[ci], myw, newWord, lane);
+    } else {
+      // ---- sparse group: queue its unvisited vertices
+      if (listCount + total > BU_LIST) run_batch(BU_BATCH);
+      uint32_t at = listCount + incl - cnt;
+      for (uint32_t bits = unvw; bits; bits &= bits - 1) {
+        const uint32_t u = myw * 32u + (uint32_t)(__ffs(bits) - 1);
+        list[at++] = u;
+        prefetch_l2(&p.head[u]);
+      }
+      listCount += total;
+      __syncwarp();
+      if (listCount >= BU_BATCH) run_batch(BU_BATCH);
+    }
+  }
+  while (listCount) run_batch(min(listCount, BU_BATCH));
   wl_flush(sh, WLn, &ctrl->wlc[ci]);
   block_accumulate(sh, c, ctrl, ci);
 }
 
-// Direction of level `level` (PAPER.md Eq. 6 analogue; DESIGN.md "Switch").  All threads evaluate it on the same
+// Direction of level `level` (PAPER.md Eq. 6 analogue; DESIGN.md §5.4).  All threads evaluate it on the same
 // counters, so the decision is grid-uniform.
 __device__ __forceinline__ bool choose_bottom_up(const BfsParams& p, uint32_t level, unsigned long long nf,
                                                  unsigned long long mf, unsigned long long nu, unsigned long long mu) {
-  if (p.switching == 2) return true;
+  if (p.switching == 2) return level >= 2;
   if (p.switching == 5) return (p.buMask >> min(level, 31u)) & 1u;
   if (p.switching != 0) return false;
-  // bytes each direction is expected to move: top-down reads every edge out of the frontier; bottom-up sweeps the
-  // visited bitmap, reads the row pointers and first neighbours of every unvisited vertex and a fraction of the
-  // remaining unvisited edges
-  const float costTd = 4.0f * (float)mf + 32.0f * (float)nf;
-  const float costBu = 12.0f * (float)p.nSweepWords + 48.0f * (float)nu + 0.5f * (float)mu;
+  // Top-down examines every edge out of the frontier (one bitmap probe each) and sweeps the bitmaps once.
+  // Bottom-up examines, for every unvisited vertex, neighbours until the first one in the frontier: with a fraction
+  // mf/nnz of all edge endpoints in the frontier that is about nnz/mf per vertex, and never more than its degree.
+  const float fmf = (float)mf, fnu = (float)nu;
+  const float perVertex = fminf((float)p.nnz / fmaxf(fmf, 1.0f), fnu > 0.f ? (float)mu / fnu : 0.f);
+  const float costTd = p.cTdEdge * fmf + p.cTdVertex * (float)nf + p.cTdWord * (float)p.nSweepWords;
+  const float costBu = p.cBuVertex * fnu + p.cBuScan * fnu * perVertex + p.cBuWord * (float)p.nSweepWords;
   return costBu * 10.0f < p.eta * costTd;
 }
 
 template <int CONTR>
 __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid_constant__ BfsParams p) {
-  __shared__ LazyShared sh;
+  extern __shared__ __align__(16) unsigned char lazy_smem[];
+  LazyShared& sh = *reinterpret_cast<LazyShared*>(lazy_smem);
   unsigned int epoch = 0;
   Ctrl* ctrl = p.ctrl;
   const uint64_t gtid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (uint64_t)gridDim.x * blockDim.x;
@@ -421,20 +783,30 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
   if (threadIdx.x == 0) sh.wlCnt = 0;
   if (leader) ctrl->t0 = globaltimer();
 
-  // A4 per-call init: bitmaps cleared, V = F_curr = {src}.  The level array is NOT initialised:
-  // it is written once per discovered vertex and read only where V is set (hand-off below).
+  // A4 per-call init: bitmaps cleared, V = F_curr = {src}; levels_out = -1 everywhere.
   const uint32_t nSW = p.nSweepWords, srcWord = p.src >> 5, srcBit = 1u << (p.src & 31u);
-  for (uint64_t i = gtid; i < nSW; i += nth) {
+  const uint32_t nClear = (nSW + 7u) & ~7u;  // the bottom-up step reads 8 words at a time (buffers are padded)
+  for (uint64_t i = gtid; i < nClear; i += nth) {
     const uint32_t x = (i == srcWord) ? srcBit : 0u;
     p.V[i] = x;
     p.F[0][i] = x;
     p.F[1][i] = 0;
     p.F[2][i] = 0;
   }
+  {
+    uint32_t* o = reinterpret_cast<uint32_t*>(p.out);
+    const uint64_t head = min((uint64_t)p.n, (uint64_t)((16u - ((uintptr_t)o & 15u)) & 15u) >> 2);
+    const uint64_t n4 = ((uint64_t)p.n - head) >> 2;
+    uint4* o4 = reinterpret_cast<uint4*>(o + head);
+    const uint4 m1 = make_uint4(NONE, NONE, NONE, NONE);
+    for (uint64_t i = gtid; i < n4; i += nth) o4[i] = m1;
+    const uint64_t tail0 = head + (n4 << 2);
+    if (gtid < head) o[gtid] = NONE;
+    if (gtid < (uint64_t)p.n - tail0) o[tail0 + gtid] = NONE;
+  }
   const uint32_t srcDeg = __ldg(&p.rowptr[p.src + 1]) - __ldg(&p.rowptr[p.src]);
   if (leader) {
-    // level 0: the source itself (L[src] = 0, frontier = {src})
-    p.L[p.src] = 0;
+    // level 0: the source itself (frontier = {src})
     p.WL[0][0] = srcWord;
     ctrl->wlc[0] = 1;
     ctrl->newcount[0] = 1;
@@ -442,16 +814,29 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     ctrl->unvisited[0] = (unsigned long long)min((uint64_t)p.n, (uint64_t)nSW * 32u) - 1u;
   }
   grid_barrier(&ctrl->bar, epoch);
+  if (leader) {
+    p.out[p.srcOrig] = 0;  // L[src] = 0 (after the fill: ordered by the barrier)
+    ctrl->tInit = globaltimer() - ctrl->t0;
+  }
 
   unsigned long long degVisited = 0;  // sum of degrees of all visited vertices
   uint32_t level = 1;
   for (;; ++level) {
     const uint32_t cp = (level - 1) % 3u, ci = level % 3u, cn = (level + 1) % 3u;
-    const unsigned long long nf = ld_volatile(&ctrl->newcount[cp]);
+    // one thread per CTA reads the level's control words (every warp reading them would queue on one L2 slice)
+    if (threadIdx.x == 0) {
+      sh.ctl[0] = ld_volatile(&ctrl->newcount[cp]);
+      sh.ctl[1] = ld_volatile(&ctrl->mf[cp]);
+      sh.ctl[2] = ld_volatile(&ctrl->unvisited[cp]);
+      sh.ctl[3] = ld_volatile(&ctrl->wlc[cp]);
+    }
+    __syncthreads();
+    const unsigned long long nf = sh.ctl[0];
+    const unsigned long long mf = sh.ctl[1];
+    const unsigned long long unvAll = sh.ctl[2];
+    const uint32_t wlCount = (uint32_t)sh.ctl[3];
+    __syncthreads();
     if (nf == 0) break;  // empty frontier ("terminates at the first level with x = 0")
-    const unsigned long long mf = ld_volatile(&ctrl->mf[cp]);
-    const unsigned long long unvAll = ld_volatile(&ctrl->unvisited[cp]);
-    const uint32_t wlCount = ld_volatile(&ctrl->wlc[cp]);
     degVisited += mf;
     const unsigned long long nu = unvAll > p.nIsoInSweep ? unvAll - p.nIsoInSweep : 0ull;
     const unsigned long long mu = p.nnz > degVisited ? p.nnz - degVisited : 0ull;
@@ -471,17 +856,18 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     }
     unsigned long long tStage1 = 0;
     if (bottomUp) {
-      bu_level(p, sh, level, Fp, Fn, Fs, p.WL[level & 1u], ctrl, ci);
+      bu_level(p, sh, level, Fp, Fn, Fs, p.WL[level & 1u], ctrl, ci, nu);
       grid_barrier(&ctrl->bar, epoch);
       if (leader) tStage1 = globaltimer();
     } else {
       td_phase_a<CONTR>(p, sh, p.WL[(level - 1) & 1u], wlCount, Fp, Fn, ctrl, ci);
       grid_barrier(&ctrl->bar, epoch);
-      const uint32_t nBig = ld_volatile(&ctrl->nBig[ci]);
-      if (nBig) {  // hubs: cut into equal chunks, spread over the grid
-        td_phase_b1(p, min(nBig, p.recCap));
-        grid_barrier(&ctrl->bar, epoch);
-        td_phase_b2<CONTR>(p, min(ld_volatile(&ctrl->qc[ci]), p.chunkCap), Fp, Fn);
+      if (threadIdx.x == 0) sh.ctl[0] = ld_volatile(&ctrl->qc[ci]);
+      __syncthreads();
+      const uint32_t nChunks = (uint32_t)sh.ctl[0];
+      __syncthreads();
+      if (nChunks) {  // hubs: equal chunks spread over the grid
+        td_phase_b<CONTR>(p, min(nChunks, p.chunkCap), Fn);
         grid_barrier(&ctrl->bar, epoch);
       }
       if (leader) tStage1 = globaltimer();
@@ -505,22 +891,6 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     }
   }
   if (leader) ctrl->nlevels = level - 1;
-
-  // A10 hand-off: levels in original ids, -1 = unreachable ("infinity"; reading R1)
-  if (p.perm) {
-    for (uint64_t v = gtid; v < p.n; v += nth) {
-      const uint32_t pv = __ldg(&p.perm[v]);
-      int32_t r = -1;
-      if ((pv >> 5) < nSW && ((p.V[pv >> 5] >> (pv & 31u)) & 1u)) r = p.L[pv];
-      p.out[v] = r;
-    }
-  } else {
-    for (uint64_t v = gtid; v < p.n; v += nth) {
-      const uint32_t w = (uint32_t)(v >> 5);
-      const bool vis = w < nSW && ((p.V[w] >> (v & 31u)) & 1u);
-      if (!vis) p.out[v] = -1;
-    }
-  }
 }
 
 __global__ void isolated_source_kernel(int32_t* out, uint32_t n, uint32_t src) {
@@ -533,14 +903,15 @@ int coop_blocks(K kernel) {
   int dev = 0, sms = 0, perSm = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&perSm, kernel, BLOCK_THREADS, 0) != cudaSuccess) return 0;
+  if (cudaFuncSetAttribute((const void*)kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LazyShared)) != cudaSuccess) return 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&perSm, kernel, BLOCK_THREADS, sizeof(LazyShared)) != cudaSuccess) return 0;
   return sms * (perSm > 0 ? 1 : 0);  // one CTA per SM: the cheapest grid barrier
 }
 
 template <class K>
 cudaError_t coop_launch(K kernel, const BfsParams& p, int gridBlocks, cudaStream_t st) {
   void* args[] = {(void*)&p};
-  return cudaLaunchCooperativeKernel((const void*)kernel, dim3(gridBlocks), dim3(BLOCK_THREADS), args, 0, st);
+  return cudaLaunchCooperativeKernel((const void*)kernel, dim3(gridBlocks), dim3(BLOCK_THREADS), args, sizeof(LazyShared), st);
 }
 
 }  // namespace
@@ -561,6 +932,9 @@ cudaError_t launch_isolated_source(int32_t* out, uint32_t n, uint32_t src, cudaS
   return cudaGetLastError();
 }
 
-int max_coop_blocks_lazy() { return coop_blocks(bfs_lazy_kernel<2>); }
+int max_coop_blocks_lazy() {  // also opts every instantiation into the dynamic shared-memory size
+  const int a = coop_blocks(bfs_lazy_kernel<1>), b = coop_blocks(bfs_lazy_kernel<2>), c = coop_blocks(bfs_lazy_kernel<3>);
+  return std::min(a, std::min(b, c));
+}
 
 }  // namespace blest

@@ -28,6 +28,7 @@ struct Ctrl {
   unsigned long long mf[4];         // sum of degrees of the vertices discovered at this level
   unsigned long long buScanned[4];  // neighbours scanned by the bottom-up stage
   unsigned long long t0;            // %globaltimer at kernel start
+  unsigned long long tInit;         // lazy kernel: ns from kernel start to the end of the per-call init
   unsigned int wlc[4];              // lazy kernel: frontier word-list lengths (rotating, level mod 3)
   unsigned int nBig[4];             // lazy kernel: deferred big segments of the level (rotating)
 };
