@@ -1,0 +1,97 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (same Graph options, same
+sources): levels compared element by element with the oracle for a few sources per config (the oracle finishes one
+BFS in seconds), plus integer farness / reach of further sources (bit-exact).  Config 5: closeness of ALL vertices on
+the GPU, compared on a seeded sample of sources the oracle computes one by one."""
+import numpy as np
+import pytest
+
+import graphgen as gg
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+# reorder as in bench.py (REORDER_FOR); number of sources compared element-wise / by (far, reach)
+FULL = {
+    "c2_grid4096": dict(reorder="none", n_levels=2, n_far=2),
+    "c3_gnm25": dict(reorder="none", n_levels=2, n_far=4),
+    "c4_rmat24": dict(reorder="degree", n_levels=3, n_far=8),
+}
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+
+    import paper_2606_05081_b200 as blest
+
+    assert torch.cuda.is_available()
+    blest.load()
+    return torch, blest
+
+
+@pytest.mark.parametrize("name", sorted(FULL))
+def test_full_size_levels_and_farness(env, name):
+    torch, blest = env
+    cfg = FULL[name]
+    n, rp, ci = gg.make_config(name)
+    srcs = gg.config_sources(name, rp)
+    out = torch.empty(n, dtype=torch.int32, device="cuda")
+    with blest.Graph(n, rp, ci, reorder=cfg["reorder"]) as g:
+        for s in srcs[: cfg["n_levels"]]:
+            g.bfs(int(s), out)
+            got = out.cpu().numpy()
+            want = oracle.bfs(n, rp, ci, int(s))
+            bad = np.flatnonzero(got != want)
+            assert bad.size == 0, f"{name} src {int(s)}: {bad.size} mismatches, first {bad[:5]}"
+            g.trace()  # surfaces a work-queue overflow
+        more = srcs[cfg["n_levels"]: cfg["n_levels"] + cfg["n_far"]]
+        if more.size:
+            far_w, reach_w, _, _ = oracle.closeness(n, rp, ci, more)
+            for s, fw, rw in zip(more, far_w, reach_w):
+                g.bfs(int(s), out)
+                lv = out.cpu().numpy()
+                far, reach = oracle.farness(lv)  # plain sum / count of the GPU's level array
+                assert (far, reach) == (int(fw), int(rw)), f"{name} src {int(s)}"
+                assert lv[int(s)] == 0 and lv.min() >= -1
+
+
+def test_full_size_c3_rcm(env):
+    """Config 3 'with and without RCM reordering before BVSS build': the reordered run gives the same levels."""
+    torch, blest = env
+    n, rp, ci = gg.make_config("c3_gnm25")
+    s = int(gg.config_sources("c3_gnm25", rp)[0])
+    out = torch.empty(n, dtype=torch.int32, device="cuda")
+    with blest.Graph(n, rp, ci, reorder="rcm") as g:
+        g.bfs(s, out)
+        assert np.array_equal(out.cpu().numpy(), oracle.bfs(n, rp, ci, s))
+
+
+def test_full_size_c5_closeness_sampled(env):
+    """Config 5: all 262 144 vertices are sources (kappa = 64 batches); farness / reach bit-exact and closeness equal to
+    the oracle's IEEE division on a seeded sample of 512 sources (incl. isolated vertices)."""
+    torch, blest = env
+    n, rp, ci = gg.make_config("c5_rmat18")
+    rng = np.random.Generator(np.random.PCG64(5))
+    sample = np.sort(rng.choice(n, size=512, replace=False)).astype(np.uint32)
+    far_w, reach_w, cc_w, _ = oracle.closeness(n, rp, ci, sample)
+    with blest.Graph(n, rp, ci, kappa=64) as g:
+        far = torch.zeros(n, dtype=torch.int64, device="cuda")
+        reach = torch.zeros(n, dtype=torch.int32, device="cuda")
+        g.farness(far, reach)
+        cc = torch.zeros(n, dtype=torch.float64, device="cuda")
+        g.closeness(cc)
+        far_g = far.cpu().numpy().view(np.uint64)
+        reach_g = reach.cpu().numpy().view(np.uint32)
+        cc_g = cc.cpu().numpy()
+    assert np.array_equal(far_g[sample], far_w)
+    assert np.array_equal(reach_g[sample], reach_w)
+    assert np.allclose(cc_g[sample], cc_w, rtol=1e-12, atol=0.0)
+    assert np.array_equal(cc_g[sample], cc_w)
+    # properties that hold for every source: reach >= 1; far = 0 iff reach = 1; closeness in [0, 1]
+    assert reach_g.min() >= 1 and np.array_equal(far_g == 0, reach_g == 1)
+    assert cc_g.min() >= 0.0 and cc_g.max() <= 1.0
+    # sum over sources of far = sum over targets of far (undirected graph): both are the same all-pairs sum, and the
+    # component sizes agree: every vertex of a component reports the same reach
+    lv = oracle.bfs(n, rp, ci, int(sample[np.argmax(reach_w)]))
+    comp = lv >= 0
+    assert np.all(reach_g[comp] == reach_g[comp][0])
