@@ -347,8 +347,9 @@ def main():
         if os.path.exists(tp):
             try:
                 t = json.load(open(tp)).get(f"{args.config}/{args.shrink}")
-                if t:
-                    line["roofline"]["traffic"] = t
+                if t:  # bytes per launch, like `achieved`'s numerator
+                    line["roofline"]["traffic"] = float(t["dram_bytes_per_launch_mean"])
+                    line["roofline"]["traffic_source"] = t["source"]
             except Exception:
                 pass
         if not args.no_cpu_baseline:
