@@ -492,8 +492,8 @@ __device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_
       }
     }
   }
-  c.qbytes += 8ull * __popc(act);
-  uint32_t found = 0;
+  c.qbytes += 8u * (uint32_t)__popc(act);
+  uint32_t found = 0, probed = 0;
   {
     uint32_t f[K];
 #pragma unroll
@@ -501,10 +501,11 @@ __device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_
 #pragma unroll
     for (int k = 0; k < K; ++k)
       if (h[k].x != NONE) {
-        ++c.scanned;
+        probed |= 1u << k;
         if ((f[k] >> (h[k].x & 31u)) & 1u) found |= 1u << k;
       }
   }
+  c.scanned += (uint32_t)__popc(probed);
   uint32_t need = 0;
 #pragma unroll
   for (int k = 0; k < K; ++k)
@@ -515,10 +516,8 @@ __device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_
     for (int k = 0; k < K; ++k) f[k] = ((need >> k) & 1u) ? Fp[(h[k].y & 0x7FFFFFFFu) >> 5] : 0u;
 #pragma unroll
     for (int k = 0; k < K; ++k)
-      if ((need >> k) & 1u) {
-        ++c.scanned;
-        if ((f[k] >> (h[k].y & 31u)) & 1u) found |= 1u << k;
-      }
+      if (((need >> k) & 1u) && ((f[k] >> (h[k].y & 31u)) & 1u)) found |= 1u << k;
+    c.scanned += (uint32_t)__popc(need);
   }
   uint32_t more = staged;
 #pragma unroll
@@ -644,8 +643,12 @@ __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uin
     for (int k = 0; k < 8; ++k) o[k] = ((found >> k) & 1u) ? (p.iperm ? __ldg(&p.iperm[u[k] & ~CSR_STAGE]) : (u[k] & ~CSR_STAGE)) : 0u;
 #pragma unroll
     for (int k = 0; k < 8; ++k) dg[k] = ((found >> k) & 1u) ? __ldg(&p.deg[u[k] & ~CSR_STAGE]) : 0u;
+    {
+      uint32_t sum = 0;
 #pragma unroll
-    for (int k = 0; k < 8; ++k) c.mf += dg[k];
+      for (int k = 0; k < 8; ++k) sum += dg[k];
+      c.mf += sum;
+    }
     batchRan = true;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
@@ -690,27 +693,18 @@ __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uin
           const uint32_t wbits = __shfl_sync(FULL, unvw, 8u * sub + k);
           u[k] = ((wbits >> lane) & 1u) ? (gw + 8u * sub + k) * 32u + lane : NONE;
         }
-#pragma unroll
-        for (int k = 0; k < 8; ++k)  // the write-back reads these: start the lines towards L2 now
-          if (u[k] != NONE) {
-            if (p.iperm) prefetch_l2(&p.iperm[u[k]]);
-            prefetch_l2(&p.deg[u[k]]);
-          }
-        if (sub + 1 < G / 8u) {  // and the heads of the next 8 words
-#pragma unroll
-          for (int k = 0; k < 8; ++k) {
-            const uint32_t wbits = __shfl_sync(FULL, unvw, (8u * sub + 8u + k) & 31u);
-            if ((wbits >> lane) & 1u) prefetch_l2(&p.head[(size_t)(gw + 8u * sub + 8u + k) * 32u + lane]);
-          }
-        }
         const uint32_t found = bu_resolve<true>(p, Fp, fshare, slotU, slotTag, lane, u, c, list, listCount);
         uint32_t o[8], dg[8];
 #pragma unroll
         for (int k = 0; k < 8; ++k) o[k] = ((found >> k) & 1u) ? (p.iperm ? __ldg(&p.iperm[u[k]]) : u[k]) : 0u;
 #pragma unroll
         for (int k = 0; k < 8; ++k) dg[k] = ((found >> k) & 1u) ? __ldg(&p.deg[u[k]]) : 0u;
+        {
+          uint32_t sum = 0;  // 8 degrees < 2^29 each
 #pragma unroll
-        for (int k = 0; k < 8; ++k) c.mf += dg[k];
+          for (int k = 0; k < 8; ++k) sum += dg[k];
+          c.mf += sum;
+        }
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
           if ((found >> k) & 1u) p.out[o[k]] = (int32_t)level;  // lane = bit: coalesced when there is no reordering
