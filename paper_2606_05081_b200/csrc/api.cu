@@ -54,6 +54,7 @@ struct blest_graph {
   std::vector<uint64_t> setDeg;    // per slice set: degree sum of its 8 columns
   uint2* dHead = nullptr;
   uint32_t* dDeg = nullptr;
+  uint32_t* dIso = nullptr;
   uint16_t* dPopThr = nullptr;
   std::vector<uint32_t> isoBits;  // host bitmap of zero-degree vertices (internal ids): such a source reaches nothing
   uint32_t *dV = nullptr, *dF[3] = {nullptr, nullptr, nullptr}, *dWL[2] = {nullptr, nullptr};
@@ -315,6 +316,8 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
         }
         if ((rc = dev_alloc(g, &g->dHead, g->n))) return rc;
         if ((rc = dev_alloc(g, &g->dDeg, g->n))) return rc;
+        if ((rc = dev_alloc(g, &g->dIso, (uint64_t)g->nwords + 16, true))) return rc;
+        CK(cudaMemcpy(g->dIso, g->isoBits.data(), (size_t)g->nwords * 4, cudaMemcpyHostToDevice));
         if ((rc = dev_alloc(g, &g->dPopThr, (uint64_t)g->nwords + 16))) return rc;
         CK(cudaMemcpy(g->dHead, head.data(), (size_t)g->n * sizeof(uint2), cudaMemcpyHostToDevice));
         CK(cudaMemcpy(g->dDeg, deg.data(), (size_t)g->n * 4, cudaMemcpyHostToDevice));
@@ -422,7 +425,7 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
   p.rowptr = h->dRowptr; p.colidx = h->dColidx;
   p.perm = h->hasPerm ? h->dPerm : nullptr;
   p.iperm = h->hasPerm ? h->dIperm : nullptr;
-  p.nSweepWords = h->nSweepWords; p.nIsoInSweep = h->nIsoInSweep;
+  p.nSweepWords = h->nSweepWords; p.nIsoInSweep = h->nIsoInSweep; p.isoBits = h->dIso;
   p.V = h->dV; p.F[0] = h->dF[0]; p.F[1] = h->dF[1]; p.F[2] = h->dF[2];
   p.WL[0] = h->dWL[0]; p.WL[1] = h->dWL[1];
   p.chunks = h->dChunks; p.chunkCap = h->chunkCap;

@@ -13,6 +13,7 @@ namespace {
 struct SharedScratch {
   BigSeg bigList[WARPS_PER_BLOCK][BIG_CAP];
   uint32_t bigCnt[WARPS_PER_BLOCK];
+  uint32_t qcount;  // queue length of the level, read by one thread and broadcast
 };
 
 // Fill an int32/uint32 array of exactly `count` words with `value`, except index `special` which gets `sval`.
@@ -64,7 +65,11 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_eager_kernel(const __gri
 
   uint32_t level = 1;
   for (;; ++level) {
-    const uint32_t qcount = ld_volatile(&ctrl->qc[level % 3u]);
+    // one thread per CTA reads the queue length (every warp reading it would queue on one L2 slice)
+    if (threadIdx.x == 0) sh.qcount = ld_volatile(&ctrl->qc[level % 3u]);
+    __syncthreads();
+    const uint32_t qcount = sh.qcount;
+    __syncthreads();
     if (qcount == 0) break;
     const uint2* Qc = p.Q[level & 1u];
     uint2* Qn = p.Q[(level + 1) & 1u];
@@ -88,19 +93,33 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_eager_kernel(const __gri
       const uint32_t hits = contract<CONTR>(m, alpha, lane);
       uint32_t segA[4], segN[4], segS[4], nseg = 0, cnt = 0;
       const uint32_t ru[4] = {rows.x, rows.y, rows.z, rows.w};
+      // the level of every row that hit, and (speculatively) the quad range of its slice set, in one round of loads
+      int lu[4];
+      uint32_t sa[4], sb[4];
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
+        lu[c] = 0;
+        sa[c] = sb[c] = 0;
         if ((hits >> c) & 1u) {
-          const uint32_t u = ru[c];
-          if (p.L[u] < 0) {         // "if l < L[u]"; benign same-value race
-            p.L[u] = (int32_t)level;
-            const uint32_t so = u >> 3;
-            const int old = atomicMax(&p.stamp[so], (int)level);  // PAPER.md:302-305 "old = 0": first to activate the set
-            if (old < (int)level) {
-              const uint32_t a = __ldg(&p.setPtr[so]), q = __ldg(&p.setPtr[so + 1]) - a;
-              if (q) { segA[nseg] = a; segN[nseg] = q; segS[nseg] = so; ++nseg; cnt += seg_entries(0, q); }
-            }
-          }
+          lu[c] = p.L[ru[c]];
+          sa[c] = __ldg(&p.setPtr[ru[c] >> 3]);
+          sb[c] = __ldg(&p.setPtr[(ru[c] >> 3) + 1]);
+        }
+      }
+      int old[4];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        old[c] = (int)level;
+        if (((hits >> c) & 1u) && lu[c] < 0) {  // "if l < L[u]"; benign same-value race
+          p.L[ru[c]] = (int32_t)level;
+          old[c] = atomicMax(&p.stamp[ru[c] >> 3], (int)level);  // PAPER.md:302-305 "old = 0": first to activate the set
+        }
+      }
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        if (old[c] < (int)level) {
+          const uint32_t q = sb[c] - sa[c];
+          if (q) { segA[nseg] = sa[c]; segN[nseg] = q; segS[nseg] = ru[c] >> 3; ++nseg; cnt += seg_entries(0, q); }
         }
       }
       bool ok;

@@ -29,6 +29,8 @@ struct BfsParams {
   // lazy kernel state
   uint32_t nSweepWords;    // 32-vertex words covering every vertex of non-zero degree
   uint32_t nIsoInSweep;    // zero-degree vertices inside the sweep range
+  const uint32_t* isoBits; // bitmap of zero-degree vertices (padded like V): they start out "visited" so that no
+                           // sweep ever examines them; levels_out keeps their -1
   uint32_t* V;             // visited bitmap (single copy)
   uint32_t* F[3];          // frontier bitmaps, rotating: level l reads F[(l-1)%3], writes F[l%3], clears F[(l+1)%3]
   uint32_t* WL[2];         // frontier word lists (ids of non-zero words of the frontier bitmap), level parity

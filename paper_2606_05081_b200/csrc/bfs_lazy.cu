@@ -782,7 +782,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
   const uint32_t nClear = (nSW + 7u) & ~7u;  // the bottom-up step reads 8 words at a time (buffers are padded)
   for (uint64_t i = gtid; i < nClear; i += nth) {
     const uint32_t x = (i == srcWord) ? srcBit : 0u;
-    p.V[i] = x;
+    p.V[i] = x | __ldg(&p.isoBits[i]);
     p.F[0][i] = x;
     p.F[1][i] = 0;
     p.F[2][i] = 0;
@@ -805,7 +805,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     ctrl->wlc[0] = 1;
     ctrl->newcount[0] = 1;
     ctrl->mf[0] = srcDeg;
-    ctrl->unvisited[0] = (unsigned long long)min((uint64_t)p.n, (uint64_t)nSW * 32u) - 1u;
+    ctrl->unvisited[0] = (unsigned long long)min((uint64_t)p.n, (uint64_t)nSW * 32u) - 1u - p.nIsoInSweep;
   }
   grid_barrier(&ctrl->bar, epoch);
   if (leader) {
@@ -832,7 +832,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     __syncthreads();
     if (nf == 0) break;  // empty frontier ("terminates at the first level with x = 0")
     degVisited += mf;
-    const unsigned long long nu = unvAll > p.nIsoInSweep ? unvAll - p.nIsoInSweep : 0ull;
+    const unsigned long long nu = unvAll;  // zero-degree vertices count as visited from the start
     const unsigned long long mu = p.nnz > degVisited ? p.nnz - degVisited : 0ull;
     const bool bottomUp = choose_bottom_up(p, level, nf, mf, nu, mu);
     const uint32_t* Fp = p.F[cp];
@@ -877,7 +877,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       r.q_bytes = ld_volatile(&ctrl->qbytes[ci]);
       r.bu_scanned = ld_volatile(&ctrl->buScanned[ci]);
       const unsigned long long ua = ld_volatile(&ctrl->unvisited[ci]);
-      r.unvisited = (uint32_t)(ua + ((unsigned long long)p.n - min((uint64_t)p.n, (uint64_t)nSW * 32u)));
+      r.unvisited = (uint32_t)(ua + p.nIsoInSweep + ((unsigned long long)p.n - min((uint64_t)p.n, (uint64_t)nSW * 32u)));
       r.reserved = bottomUp ? 0u : ld_volatile(&ctrl->nBig[ci]);
       r.t_ns = globaltimer() - ctrl->t0;
       r.t_stage1_ns = tStage1 - ctrl->t0;

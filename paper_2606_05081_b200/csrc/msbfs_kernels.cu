@@ -20,6 +20,7 @@ struct MsShared {
   BigSeg bigList[WARPS_PER_BLOCK][BIG_CAP];
   uint32_t bigCnt[WARPS_PER_BLOCK];
   unsigned long long acc;
+  unsigned long long ctl[2];  // control words of the level, read by one thread and broadcast
   uint32_t perSource[128];
 };
 
@@ -193,8 +194,16 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_co
     grid_barrier(&ctrl->bar, epoch);
     for (uint32_t level = 1;; ++level) {
       const uint32_t pp = (level - 1) & 1u, par = level & 1u;
-      if (ld_volatile(&ctrl->newcount[pp]) == 0) break;
-      const uint32_t qcount = ld_volatile(&ctrl->qc[par]);
+      // one thread per CTA reads the control words (every warp reading them would queue on one L2 slice)
+      if (threadIdx.x == 0) {
+        sh.ctl[0] = ld_volatile(&ctrl->newcount[pp]);
+        sh.ctl[1] = ld_volatile(&ctrl->qc[par]);
+      }
+      __syncthreads();
+      const unsigned long long nnewPrev = sh.ctl[0];
+      const uint32_t qcount = (uint32_t)sh.ctl[1];
+      __syncthreads();
+      if (nnewPrev == 0) break;
       ms_stage1<KW>(p, p.Q[par], qcount);
       grid_barrier(&ctrl->bar, epoch);
       if (blockIdx.x == 0 && threadIdx.x == 0) {
