@@ -31,7 +31,7 @@ static thread_local int g_lastCuda = 0;
 static constexpr uint32_t TRACE_CAP = 1u << 17;
 static constexpr double UDIV_THRESHOLD = 25000.0;
 // switch cost model defaults, picoseconds per unit
-static constexpr float COST_TD_EDGE = 8.0f, COST_TD_VERTEX = 40.0f, COST_TD_WORD = 30.0f;
+static constexpr float COST_TD_EDGE = 14.0f, COST_TD_VERTEX = 40.0f, COST_TD_WORD = 30.0f;
 static constexpr float COST_BU_VERTEX = 4.0f, COST_BU_SCAN = 6.0f, COST_BU_WORD = 20.0f;
 
 struct blest_graph {

@@ -81,6 +81,24 @@ def test_small_graphs_default_policy(blest, torch_cuda, name, kernel):
         check_bfs(blest, torch_cuda, g, graph, sources_for(graph[0], graph[1]))
 
 
+@pytest.mark.parametrize("name", sorted(SMALL))
+def test_small_graphs_eager_grid_wide_only(blest, torch_cuda, name):
+    """Alg. 2 proper: switching="off" keeps the eager kernel on the grid-wide slice path (no small-frontier mode)."""
+    graph = SMALL[name]()
+    with blest.Graph(*graph, kernel="eager", switching="off") as g:
+        check_bfs(blest, torch_cuda, g, graph, sources_for(graph[0], graph[1]))
+
+
+@pytest.mark.parametrize("maker", [lambda: gg.gnm(200_000, 800_000, 3), lambda: gg.rmat(15, 16, 4), lambda: gg.grid2d(300, 700, 0.05, 6)])
+def test_eager_mode_transitions(blest, torch_cuda, maker):
+    """Frontiers that outgrow the single-CTA small-frontier mode (shared queue overflow, refusal) and shrink back into it."""
+    graph = maker()
+    with blest.Graph(*graph, kernel="eager") as g:
+        check_bfs(blest, torch_cuda, g, graph, sources_for(graph[0], graph[1], 3))
+        modes = set(int(m) for m in g.trace()["mode"])
+        assert modes <= {2, 3}
+
+
 @pytest.mark.parametrize("name", ["star_hub", "union", "ragged", "rmat12", "grid"])
 @pytest.mark.parametrize("switching", ["auto", "off", "bottom_up", "top_down", "slice"])
 def test_policy_independence_lazy(blest, torch_cuda, name, switching):
