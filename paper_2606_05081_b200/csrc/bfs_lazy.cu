@@ -118,8 +118,18 @@ __device__ __forceinline__ void prefetch_l2(const void* ptr) { asm volatile("pre
 // ---- lazy marks ----------------------------------------------------------------------------------
 // U candidate vertices per lane: filtered no-return atomic ORs into the next frontier.  The probes of the U
 // candidates are issued together (V first: it does not change during Stage 1, so L1 may serve it; then F_next at L2).
+// probeFn: also read F_next before the atomic.  It pays when a level has many more edges than unvisited vertices
+// (most marks would repeat an earlier one, and repeated atomics on a hot word serialise in L2); otherwise it is one
+// more scattered access per edge for nothing, so the level decides (mf > 4 nu).
+struct Marks {
+  const uint32_t* V;
+  uint32_t* Fn;
+  bool probeFn;
+};
 template <int U>
-__device__ __forceinline__ void mark_batch(const uint32_t* V, uint32_t* Fn, const uint32_t (&v)[U], uint32_t valid) {
+__device__ __forceinline__ void mark_batch(const Marks& mk, const uint32_t (&v)[U], uint32_t valid) {
+  const uint32_t* V = mk.V;
+  uint32_t* Fn = mk.Fn;
   uint32_t vw[U];
 #pragma unroll
   for (int j = 0; j < U; ++j) vw[j] = ((valid >> j) & 1u) ? V[v[j] >> 5] : FULL;
@@ -127,6 +137,12 @@ __device__ __forceinline__ void mark_batch(const uint32_t* V, uint32_t* Fn, cons
 #pragma unroll
   for (int j = 0; j < U; ++j)
     if (!((vw[j] >> (v[j] & 31u)) & 1u)) need |= 1u << j;
+  if (!mk.probeFn) {
+#pragma unroll
+    for (int j = 0; j < U; ++j)
+      if ((need >> j) & 1u) atomicOr(&Fn[v[j] >> 5], 1u << (v[j] & 31u));
+    return;
+  }
   uint32_t fw[U];
 #pragma unroll
   for (int j = 0; j < U; ++j) fw[j] = ((need >> j) & 1u) ? __ldcg(&Fn[v[j] >> 5]) : FULL;
@@ -147,7 +163,7 @@ __device__ __forceinline__ uint32_t find_owner(uint32_t incl, uint32_t idx) {
 }
 
 // CUDA-core top-down: each lane owns one adjacency segment [r0, r0+deg); the warp walks the concatenation.
-__device__ __forceinline__ void expand_edges(const BfsParams& p, uint32_t* Fn, uint32_t r0, uint32_t deg, uint32_t lane) {
+__device__ __forceinline__ void expand_edges(const BfsParams& p, const Marks& Fn, uint32_t r0, uint32_t deg, uint32_t lane) {
   const uint32_t incl = warp_incl_scan(deg, lane);
   const uint32_t total = __shfl_sync(FULL, incl, 31);
   const uint32_t basePtr = r0 - (incl - deg);
@@ -164,12 +180,12 @@ __device__ __forceinline__ void expand_edges(const BfsParams& p, uint32_t* Fn, u
         valid |= 1u << j;
       }
     }
-    mark_batch<4>(p.V, Fn, v, valid);
+    mark_batch<4>(Fn, v, valid);
   }
 }
 
 // One contiguous run of edges handled by the whole warp (balanced phase, long adjacency lists).
-__device__ __forceinline__ void warp_edges(const BfsParams& p, uint32_t* Fn, uint32_t e0, uint32_t e1, uint32_t lane) {
+__device__ __forceinline__ void warp_edges(const BfsParams& p, const Marks& Fn, uint32_t e0, uint32_t e1, uint32_t lane) {
   for (uint32_t base = e0; base < e1; base += 128u) {
     uint32_t v[4], valid = 0;
 #pragma unroll
@@ -181,20 +197,20 @@ __device__ __forceinline__ void warp_edges(const BfsParams& p, uint32_t* Fn, uin
         valid |= 1u << j;
       }
     }
-    mark_batch<4>(p.V, Fn, v, valid);
+    mark_batch<4>(Fn, v, valid);
   }
 }
 
-__device__ __forceinline__ void mark_quad(const BfsParams& p, uint32_t* Fn, const uint4& r, uint32_t hits) {
+__device__ __forceinline__ void mark_quad(const BfsParams& p, const Marks& Fn, const uint4& r, uint32_t hits) {
   const uint32_t v[4] = {r.x, r.y, r.z, r.w};
-  mark_batch<4>(p.V, Fn, v, hits);
+  mark_batch<4>(Fn, v, hits);
 }
 
 // Pull contraction over quads [a, a+nq) of ONE slice set with frontier word alpha: per lane a
 // 128-bit row-id load and a 32-bit mask load, four quads in flight.  alpha is warp-uniform, all 32 lanes take part
 // (the MMA forms of the contraction need both).
 template <int CONTR>
-__device__ __forceinline__ void warp_slices(const BfsParams& p, uint32_t* Fn, uint32_t a, uint32_t nq, uint32_t alpha,
+__device__ __forceinline__ void warp_slices(const BfsParams& p, const Marks& Fn, uint32_t a, uint32_t nq, uint32_t alpha,
                                             uint32_t lane) {
   for (uint32_t base = 0; base < nq; base += 128u) {
     uint4 r[4];
@@ -221,7 +237,7 @@ __device__ __forceinline__ void warp_slices(const BfsParams& p, uint32_t* Fn, ui
 
 // Slice path, flattened: each lane owns the quads [a, a+nq) of one slice set with its own frontier word alpha; the
 // warp walks the concatenation, two quads per lane in flight (ALU contraction: it needs no warp-uniform alpha).
-__device__ __forceinline__ void expand_slices(const BfsParams& p, uint32_t* Fn, uint32_t a, uint32_t nq, uint32_t alpha,
+__device__ __forceinline__ void expand_slices(const BfsParams& p, const Marks& Fn, uint32_t a, uint32_t nq, uint32_t alpha,
                                               uint32_t lane) {
   const uint32_t incl = warp_incl_scan(nq, lane);
   const uint32_t total = __shfl_sync(FULL, incl, 31);
@@ -253,8 +269,10 @@ __device__ __forceinline__ void expand_slices(const BfsParams& p, uint32_t* Fn, 
 // A hub segment (long adjacency list / big slice set) is cut into equal chunks by the warp that found it; the chunks
 // are consumed by the whole grid in the balanced phase.
 __device__ __forceinline__ void emit_chunks(const BfsParams& p, Ctrl* ctrl, uint32_t ci, uint32_t type, uint32_t start,
-                                            uint32_t count, uint32_t alpha, uint32_t lane) {
-  const uint32_t per = type ? CHUNK_EDGES : CHUNK_QUADS;
+                                            uint32_t count, uint32_t alpha, uint32_t lane, bool coarse) {
+  // fine chunks when the frontier is short (a few hubs must still spread over all warps), four times coarser when it
+  // is long (enough chunks anyway; a full 128-quad / 512-edge step per lane batch)
+  const uint32_t per = (type ? CHUNK_EDGES : CHUNK_QUADS) * (coarse ? 4u : 1u);
   const uint32_t nent = (count + per - 1) / per;
   uint32_t pos = 0;
   if (lane == 0) {
@@ -272,13 +290,14 @@ __device__ __forceinline__ void emit_chunks(const BfsParams& p, Ctrl* ctrl, uint
 // Stage 1, top-down, phase A: 32 non-zero frontier words per warp step (lane = word).
 template <int CONTR>
 __device__ __forceinline__ void td_phase_a(const BfsParams& p, LazyShared& sh, const uint32_t* WLc, uint32_t wlCount,
-                                           const uint32_t* Fp, uint32_t* Fn, Ctrl* ctrl, uint32_t ci) {
+                                           const uint32_t* Fp, const Marks& Fn, Ctrl* ctrl, uint32_t ci) {
   const uint32_t lane = threadIdx.x & 31;
   const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
   const int sw = p.switching;
   // words per warp step: 32 when the list is long; fewer when it is short, so that a small frontier still spreads
   // over the grid (one word per warp below nwarps words)
   const uint32_t W = min(32u, max(1u, (wlCount + nwarps - 1) / nwarps));
+  const bool coarse = wlCount >= nwarps;
   Counters c;
   for (uint32_t i0 = gwarp * W; i0 < wlCount; i0 += nwarps * W) {
     const uint32_t i = i0 + lane;
@@ -329,7 +348,7 @@ __device__ __forceinline__ void td_phase_a(const BfsParams& p, LazyShared& sh, c
           const int src = __ffs(big) - 1;
           big &= big - 1;
           const uint32_t A = __shfl_sync(FULL, a[k], src), NQ = __shfl_sync(FULL, nq[k], src), AL = __shfl_sync(FULL, alpha, src);
-          if (NQ > BIG_QUADS) emit_chunks(p, ctrl, ci, 0u, A, NQ, AL, lane);
+          if (NQ > BIG_QUADS) emit_chunks(p, ctrl, ci, 0u, A, NQ, AL, lane, coarse);
           else warp_slices<CONTR>(p, Fn, A, NQ, AL, lane);
         }
         if (CONTR == 1) expand_slices(p, Fn, a[k], nq[k] > BIG_QUADS ? 0u : nq[k], alpha, lane);
@@ -357,7 +376,7 @@ __device__ __forceinline__ void td_phase_a(const BfsParams& p, LazyShared& sh, c
         while (big) {
           const int src = __ffs(big) - 1;
           big &= big - 1;
-          emit_chunks(p, ctrl, ci, 1u, __shfl_sync(FULL, r0[q], src), __shfl_sync(FULL, deg[q], src), 0u, lane);
+          emit_chunks(p, ctrl, ci, 1u, __shfl_sync(FULL, r0[q], src), __shfl_sync(FULL, deg[q], src), 0u, lane, coarse);
         }
         expand_edges(p, Fn, r0[q], deg[q] > BIG_EDGES ? 0u : deg[q], lane);
       }
@@ -368,7 +387,7 @@ __device__ __forceinline__ void td_phase_a(const BfsParams& p, LazyShared& sh, c
 
 // Phase B: one warp per chunk, round-robin: every warp gets the same share of the hubs' bytes.
 template <int CONTR>
-__device__ __forceinline__ void td_phase_b(const BfsParams& p, uint32_t nChunks, uint32_t* Fn) {
+__device__ __forceinline__ void td_phase_b(const BfsParams& p, uint32_t nChunks, const Marks& Fn) {
   const uint32_t lane = threadIdx.x & 31;
   const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
   for (uint32_t i = gwarp; i < nChunks; i += nwarps) {
@@ -650,18 +669,20 @@ __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uin
       c.mf += sum;
     }
     batchRan = true;
+    uint32_t oldF[8];  // all eight returning atomics in flight before the first result is needed
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-      bool newWord = false;
-      const uint32_t uu = u[k] & ~CSR_STAGE;
+      oldF[k] = 1u;
       if ((found >> k) & 1u) {
+        const uint32_t uu = u[k] & ~CSR_STAGE, bit = 1u << (uu & 31u);
         p.out[o[k]] = (int32_t)level;
-        const uint32_t bit = 1u << (uu & 31u);
         atomicOr(&p.V[uu >> 5], bit);
-        newWord = atomicOr(&Fn[uu >> 5], bit) == 0u;  // first bit of the word in this level: the word joins the list
+        oldF[k] = atomicOr(&Fn[uu >> 5], bit);
       }
-      wl_append(sh, WLn, &ctrl->wlc[ci], uu >> 5, newWord, lane);
     }
+#pragma unroll
+    for (int k = 0; k < 8; ++k)  // first bit of a word in this level: the word joins the list
+      wl_append(sh, WLn, &ctrl->wlc[ci], (u[k] & ~CSR_STAGE) >> 5, oldF[k] == 0u, lane);
     c.nnew += __popc(found);
     c.unv -= __popc(found);
   };
@@ -787,17 +808,6 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     p.F[1][i] = 0;
     p.F[2][i] = 0;
   }
-  {
-    uint32_t* o = reinterpret_cast<uint32_t*>(p.out);
-    const uint64_t head = min((uint64_t)p.n, (uint64_t)((16u - ((uintptr_t)o & 15u)) & 15u) >> 2);
-    const uint64_t n4 = ((uint64_t)p.n - head) >> 2;
-    uint4* o4 = reinterpret_cast<uint4*>(o + head);
-    const uint4 m1 = make_uint4(NONE, NONE, NONE, NONE);
-    for (uint64_t i = gtid; i < n4; i += nth) o4[i] = m1;
-    const uint64_t tail0 = head + (n4 << 2);
-    if (gtid < head) o[gtid] = NONE;
-    if (gtid < (uint64_t)p.n - tail0) o[tail0 + gtid] = NONE;
-  }
   const uint32_t srcDeg = __ldg(&p.rowptr[p.src + 1]) - __ldg(&p.rowptr[p.src]);
   if (leader) {
     // level 0: the source itself (frontier = {src})
@@ -808,11 +818,23 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     ctrl->unvisited[0] = (unsigned long long)min((uint64_t)p.n, (uint64_t)nSW * 32u) - 1u - p.nIsoInSweep;
   }
   grid_barrier(&ctrl->bar, epoch);
-  if (leader) {
-    p.out[p.srcOrig] = 0;  // L[src] = 0 (after the fill: ordered by the barrier)
-    ctrl->tInit = globaltimer() - ctrl->t0;
-  }
+  if (leader) ctrl->tInit = globaltimer() - ctrl->t0;
 
+  // levels_out = -1 everywhere (reading R1).  Runs next to level 1's Stage 1, which keeps only a few
+  // warps busy and writes no level; the barrier after it orders the fill before every level write.
+  auto prefill_out = [&]() {
+  {
+      uint32_t* o = reinterpret_cast<uint32_t*>(p.out);
+      const uint64_t head = min((uint64_t)p.n, (uint64_t)((16u - ((uintptr_t)o & 15u)) & 15u) >> 2);
+      const uint64_t n4 = ((uint64_t)p.n - head) >> 2;
+      uint4* o4 = reinterpret_cast<uint4*>(o + head);
+      const uint4 m1 = make_uint4(NONE, NONE, NONE, NONE);
+      for (uint64_t i = gtid; i < n4; i += nth) o4[i] = m1;
+      const uint64_t tail0 = head + (n4 << 2);
+      if (gtid < head) o[gtid] = NONE;
+      if (gtid < (uint64_t)p.n - tail0) o[tail0 + gtid] = NONE;
+    }
+  };
   unsigned long long degVisited = 0;  // sum of degrees of all visited vertices
   uint32_t level = 1;
   for (;; ++level) {
@@ -850,18 +872,26 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     }
     unsigned long long tStage1 = 0;
     if (bottomUp) {
+      if (level == 1) {  // (scripted direction only)
+        prefill_out();
+        grid_barrier(&ctrl->bar, epoch);
+        if (leader) p.out[p.srcOrig] = 0;
+      }
       bu_level(p, sh, level, Fp, Fn, Fs, p.WL[level & 1u], ctrl, ci, nu);
       grid_barrier(&ctrl->bar, epoch);
       if (leader) tStage1 = globaltimer();
     } else {
-      td_phase_a<CONTR>(p, sh, p.WL[(level - 1) & 1u], wlCount, Fp, Fn, ctrl, ci);
+      if (level == 1) prefill_out();  // the stores drain while the (latency-bound) first expansion runs
+      const Marks mk{p.V, Fn, mf > 4ull * nu};
+      td_phase_a<CONTR>(p, sh, p.WL[(level - 1) & 1u], wlCount, Fp, mk, ctrl, ci);
       grid_barrier(&ctrl->bar, epoch);
+      if (level == 1 && leader) p.out[p.srcOrig] = 0;  // L[src] = 0 (after the fill: ordered by the barrier)
       if (threadIdx.x == 0) sh.ctl[0] = ld_volatile(&ctrl->qc[ci]);
       __syncthreads();
       const uint32_t nChunks = (uint32_t)sh.ctl[0];
       __syncthreads();
       if (nChunks) {  // hubs: equal chunks spread over the grid
-        td_phase_b<CONTR>(p, min(nChunks, p.chunkCap), Fn);
+        td_phase_b<CONTR>(p, min(nChunks, p.chunkCap), mk);
         grid_barrier(&ctrl->bar, epoch);
       }
       if (leader) tStage1 = globaltimer();
