@@ -80,6 +80,12 @@ def load_graph(name: str, shrink: int, rank: int, world: int):
     return n, rp, ci
 
 
+def rank_sources(srcs_all: np.ndarray, rank: int, world: int) -> np.ndarray:
+    """Replicas only: every rank traverses from ALL the config's sources (fixed per-rank work => weak
+    scaling), rotated by rank so that the ranks do not run the identical sequence at the same time."""
+    return np.roll(srcs_all, -rank * max(1, len(srcs_all) // max(world, 1)))
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
 
@@ -243,7 +249,7 @@ def main():
     srcs_all = gg.config_sources(args.config, rp)
     # replicas only: every rank traverses the full graph; rank r takes the sources rotated by r so that the ranks do
     # not run the identical sequence.  Per-rank work is fixed as N grows => weak scaling.
-    srcs = np.roll(srcs_all, -rank * max(1, len(srcs_all) // max(world, 1)))
+    srcs = rank_sources(srcs_all, rank, world)
     reorder = REORDER_FOR[args.config]
     log(f"[rank {rank}] {args.config} shrink {args.shrink}: n={n} nnz={ci.size} gen {gen_s:.1f}s; building (reorder={reorder})")
     t0 = time.perf_counter()
