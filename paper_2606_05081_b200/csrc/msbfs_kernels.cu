@@ -24,6 +24,32 @@ struct MsShared {
   uint32_t perSource[128];
 };
 
+// One kappa-bit word (KW 32-bit words, naturally aligned) moved with a single vector access.
+template <int KW>
+__device__ __forceinline__ void load_words(const uint32_t* base, uint64_t idx, uint32_t (&w)[KW]) {
+  if (KW == 1) w[0] = __ldcg(base + idx);
+  else if (KW == 2) {
+    const uint2 v = __ldcg(reinterpret_cast<const uint2*>(base) + idx);
+    w[0] = v.x; w[KW > 1 ? 1 : 0] = v.y;
+  } else {
+    const uint4 v = __ldcg(reinterpret_cast<const uint4*>(base) + idx);
+    w[0] = v.x; w[KW > 1 ? 1 : 0] = v.y; w[KW > 2 ? 2 : 0] = v.z; w[KW > 3 ? 3 : 0] = v.w;
+  }
+}
+// No-return OR of the fresh bits, 64 bits per atomic where the word is that wide.
+template <int KW>
+__device__ __forceinline__ void red_or_words(uint32_t* base, uint64_t idx, const uint32_t (&f)[KW]) {
+  if (KW == 1) {
+    if (f[0]) atomicOr(base + idx, f[0]);
+  } else {
+#pragma unroll
+    for (int h = 0; h < KW / 2; ++h) {
+      const unsigned long long v = (unsigned long long)f[2 * h] | ((unsigned long long)f[KW > 1 ? 2 * h + 1 : 0] << 32);
+      if (v) atomicOr(reinterpret_cast<unsigned long long*>(base) + idx * (KW / 2) + h, v);
+    }
+  }
+}
+
 template <int KW>
 __device__ __forceinline__ void ms_stage1(const MsParams& p, const uint2* Qc, uint32_t qcount) {
   const uint32_t lane = threadIdx.x & 31;
@@ -67,15 +93,20 @@ __device__ __forceinline__ void ms_stage1(const MsParams& p, const uint2* Qc, ui
         }
         const uint32_t u = ru[c];
         const uint64_t idx = (uint64_t)(u & 7u) * p.rho + (u >> 3);  // getVI(u, rho)
-        bool any = false;
+        uint32_t any = 0;
 #pragma unroll
-        for (int w = 0; w < KW; ++w) {
-          if (M[w]) {
-            const uint32_t fresh = M[w] & ~__ldcg(&p.Vn[idx * KW + w]);
-            if (fresh) { atomicOr(&p.Vn[idx * KW + w], fresh); any = true; }  // one RED per row
+        for (int w = 0; w < KW; ++w) any |= M[w];
+        if (any) {  // one probe and one RED per row, each a single kappa-bit access
+          uint32_t vn[KW], fresh[KW];
+          load_words<KW>(p.Vn, idx, vn);
+          any = 0;
+#pragma unroll
+          for (int w = 0; w < KW; ++w) { fresh[w] = M[w] & ~vn[w]; any |= fresh[w]; }
+          if (any) {
+            red_or_words<KW>(p.Vn, idx, fresh);
+            p.dirty[u >> 3] = 1;  // PAPER.md:583 dirtySets
           }
         }
-        if (any) p.dirty[u >> 3] = 1;  // PAPER.md:583 dirtySets
       }
     }
   }
