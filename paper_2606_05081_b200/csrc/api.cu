@@ -105,7 +105,7 @@ static int check_options(const blest_options_t& o) {
   if (o.reorder < 0 || o.reorder > 2 || o.builder < 0 || o.builder > 1) return BLEST_EINVAL;
   if (o.kernel < 0 || o.kernel > 2 || o.switching < 0 || o.switching > 5) return BLEST_EINVAL;
   if (o.contraction < 0 || o.contraction > 3) return BLEST_EINVAL;
-  if (o.kappa != 0 && o.kappa != 32 && o.kappa != 64 && o.kappa != 128) return BLEST_EINVAL;
+  if (o.kappa != 0 && o.kappa != 32 && o.kappa != 64 && o.kappa != 128 && o.kappa != 256) return BLEST_EINVAL;
   return BLEST_OK;
 }
 

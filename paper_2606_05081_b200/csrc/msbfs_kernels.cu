@@ -21,7 +21,8 @@ struct MsShared {
   uint32_t bigCnt[WARPS_PER_BLOCK];
   unsigned long long acc;
   unsigned long long ctl[2];  // control words of the level, read by one thread and broadcast
-  uint32_t perSource[128];
+  uint32_t perSource[256];
+  uint32_t fset[WARPS_PER_BLOCK][8 * 8];  // per warp: the kappa-bit frontier words of the current set's 8 columns
 };
 
 // One kappa-bit word (KW 32-bit words, naturally aligned) moved with a single vector access.
@@ -32,8 +33,11 @@ __device__ __forceinline__ void load_words(const uint32_t* base, uint64_t idx, u
     const uint2 v = __ldcg(reinterpret_cast<const uint2*>(base) + idx);
     w[0] = v.x; w[KW > 1 ? 1 : 0] = v.y;
   } else {
-    const uint4 v = __ldcg(reinterpret_cast<const uint4*>(base) + idx);
-    w[0] = v.x; w[KW > 1 ? 1 : 0] = v.y; w[KW > 2 ? 2 : 0] = v.z; w[KW > 3 ? 3 : 0] = v.w;
+#pragma unroll
+    for (int q = 0; q < KW / 4; ++q) {
+      const uint4 v = __ldcg(reinterpret_cast<const uint4*>(base) + idx * (KW / 4) + q);
+      w[KW > 3 ? 4 * q : 0] = v.x; w[KW > 3 ? 4 * q + 1 : 0] = v.y; w[KW > 3 ? 4 * q + 2 : 0] = v.z; w[KW > 3 ? 4 * q + 3 : 0] = v.w;
+    }
   }
 }
 // No-return OR of the fresh bits, 64 bits per atomic where the word is that wide.
@@ -51,7 +55,8 @@ __device__ __forceinline__ void red_or_words(uint32_t* base, uint64_t idx, const
 }
 
 template <int KW>
-__device__ __forceinline__ void ms_stage1(const MsParams& p, const uint2* Qc, uint32_t qcount) {
+__device__ __forceinline__ void ms_stage1(const MsParams& p, MsShared& sh, const uint2* Qc, uint32_t qcount) {
+  uint32_t* fset = sh.fset[threadIdx.x >> 5];
   const uint32_t lane = threadIdx.x & 31;
   const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
   for (uint32_t i = gwarp; i < qcount; i += nwarps) {
@@ -63,20 +68,16 @@ __device__ __forceinline__ void ms_stage1(const MsParams& p, const uint2* Qc, ui
       rows = __ldg(p.rowIds + e.x + lane);
       m = __ldg(p.masks + e.x + lane);
     }
-    // the first sigma lanes gather the kappa-bit frontier words of the set's 8 columns
-    uint32_t fv[KW];
-#pragma unroll
-    for (int w = 0; w < KW; ++w) fv[w] = 0;
+    // the first sigma lanes gather the kappa-bit frontier words of the set's 8 columns into shared
+    // memory; every lane then reads the words its mask bits select (same address across lanes: a broadcast)
+    __syncwarp();
     if (lane < 8) {
-      const uint64_t idx = (uint64_t)lane * p.rho + s;
+      uint32_t fv[KW];
+      load_words<KW>(p.F, (uint64_t)lane * p.rho + s, fv);
 #pragma unroll
-      for (int w = 0; w < KW; ++w) fv[w] = p.F[idx * KW + w];
+      for (int w = 0; w < KW; ++w) fset[lane * KW + w] = fv[w];
     }
-    uint32_t f[8][KW];
-#pragma unroll
-    for (int j = 0; j < 8; ++j)
-#pragma unroll
-      for (int w = 0; w < KW; ++w) f[j][w] = __shfl_sync(0xffffffffu, fv[w], j);
+    __syncwarp();
     const uint32_t ru[4] = {rows.x, rows.y, rows.z, rows.w};
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
@@ -85,11 +86,10 @@ __device__ __forceinline__ void ms_stage1(const MsParams& p, const uint2* Qc, ui
         uint32_t M[KW];  // per-row kappa-bit accumulation buffer ("M[0..3]")
 #pragma unroll
         for (int w = 0; w < KW; ++w) M[w] = 0;
+        for (uint32_t b = mb; b; b &= b - 1) {  // M = OR over the set bits j of the mask of F_curr^kappa[column j]
+          const uint32_t j = (uint32_t)__ffs(b) - 1u;
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const uint32_t sel = 0u - ((mb >> j) & 1u);
-#pragma unroll
-          for (int w = 0; w < KW; ++w) M[w] |= f[j][w] & sel;
+          for (int w = 0; w < KW; ++w) M[w] |= fset[j * KW + w];
         }
         const uint32_t u = ru[c];
         const uint64_t idx = (uint64_t)(u & 7u) * p.rho + (u >> 3);  // getVI(u, rho)
@@ -184,7 +184,7 @@ __device__ __forceinline__ void ms_stage2(const MsParams& p, MsShared& sh, uint3
     }
   }
   __syncthreads();
-  if (threadIdx.x < 128) sh.perSource[threadIdx.x] = 0;
+  if (threadIdx.x < 256) sh.perSource[threadIdx.x] = 0;
   __syncthreads();
 }
 
@@ -196,7 +196,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_co
   Ctrl* ctrl = p.ctrl;
   const uint64_t gtid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (uint64_t)gridDim.x * blockDim.x;
   if (threadIdx.x < WARPS_PER_BLOCK) sh.bigCnt[threadIdx.x] = 0;
-  if (threadIdx.x < 128) sh.perSource[threadIdx.x] = 0;
+  if (threadIdx.x < 256) sh.perSource[threadIdx.x] = 0;
   if (threadIdx.x == 0) sh.acc = 0;
   __syncthreads();
   const uint64_t stateWords = (uint64_t)p.rho * 8u * KW;
@@ -235,7 +235,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_co
       const uint32_t qcount = (uint32_t)sh.ctl[1];
       __syncthreads();
       if (nnewPrev == 0) break;
-      ms_stage1<KW>(p, p.Q[par], qcount);
+      ms_stage1<KW>(p, sh, p.Q[par], qcount);
       grid_barrier(&ctrl->bar, epoch);
       if (blockIdx.x == 0 && threadIdx.x == 0) {
         ctrl->qc[par] = 0;
@@ -287,6 +287,7 @@ cudaError_t launch_msbfs(const MsParams& p, int gridBlocks, cudaStream_t st) {
     case 32: k = (const void*)msbfs_kernel<1>; break;
     case 64: k = (const void*)msbfs_kernel<2>; break;
     case 128: k = (const void*)msbfs_kernel<4>; break;
+    case 256: k = (const void*)msbfs_kernel<8>; break;
     default: return cudaErrorInvalidValue;
   }
   return cudaLaunchCooperativeKernel(k, dim3(gridBlocks), dim3(BLOCK_THREADS), args, 0, st);
@@ -303,6 +304,6 @@ cudaError_t launch_closeness_finalize(uint32_t n, uint32_t rho, const uint32_t* 
   return cudaGetLastError();
 }
 
-int max_coop_blocks_msbfs() { return coop_blocks(msbfs_kernel<4>); }
+int max_coop_blocks_msbfs() { return std::min(coop_blocks(msbfs_kernel<4>), coop_blocks(msbfs_kernel<8>)); }
 
 }  // namespace blest

@@ -178,7 +178,7 @@ def test_configs_reduced(blest, torch_cuda, name, shrink):
 
 
 # ---- multi-source BFS (A11) and closeness (A12) ------------------------------------------------------------------
-@pytest.mark.parametrize("kappa", [32, 64, 128])
+@pytest.mark.parametrize("kappa", [32, 64, 128, 256])
 def test_msbfs_rows_equal_single_source(blest, torch_cuda, kappa):
     torch = torch_cuda
     graph = gg.disjoint_union(gg.rmat(9, 8, 11), gg.path(13), gg.empty(3))
@@ -201,7 +201,7 @@ def test_msbfs_rows_equal_single_source(blest, torch_cuda, kappa):
 
 
 @pytest.mark.parametrize("reorder", ["none", "degree"])
-@pytest.mark.parametrize("kappa", [32, 64, 128])
+@pytest.mark.parametrize("kappa", [32, 64, 128, 256])
 def test_closeness_all_vertices(blest, torch_cuda, reorder, kappa):
     torch = torch_cuda
     graph = gg.disjoint_union(gg.rmat(10, 8, 21), gg.star(30, 2), gg.empty(5), gg.path(2))
