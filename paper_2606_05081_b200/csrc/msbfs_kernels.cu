@@ -40,6 +40,17 @@ __device__ __forceinline__ void load_words(const uint32_t* base, uint64_t idx, u
     }
   }
 }
+template <int KW>
+__device__ __forceinline__ void store_words(uint32_t* base, uint64_t idx, const uint32_t (&w)[KW]) {
+  if (KW == 1) base[idx] = w[0];
+  else if (KW == 2) reinterpret_cast<uint2*>(base)[idx] = make_uint2(w[0], w[KW > 1 ? 1 : 0]);
+  else {
+#pragma unroll
+    for (int q = 0; q < KW / 4; ++q)
+      reinterpret_cast<uint4*>(base)[idx * (KW / 4) + q] =
+          make_uint4(w[KW > 3 ? 4 * q : 0], w[KW > 3 ? 4 * q + 1 : 0], w[KW > 3 ? 4 * q + 2 : 0], w[KW > 3 ? 4 * q + 3 : 0]);
+  }
+}
 // No-return OR of the fresh bits, 64 bits per atomic where the word is that wide.
 template <int KW>
 __device__ __forceinline__ void red_or_words(uint32_t* base, uint64_t idx, const uint32_t (&f)[KW]) {
@@ -127,34 +138,46 @@ __device__ __forceinline__ void ms_stage2(const MsParams& p, MsShared& sh, uint3
     if (s < p.Ns && p.dirty[s]) {  // skip slice sets nobody marked
       p.dirty[s] = 0;
       uint32_t A = 0;
+      constexpr uint32_t R = KW <= 2 ? 8u : (KW == 4 ? 4u : 2u);  // rows whose words are in flight together
 #pragma unroll
-      for (uint32_t j = 0; j < 8; ++j) {
-        const uint64_t idx = (uint64_t)j * p.rho + s;
-        uint32_t pc = 0;
+      for (uint32_t j0 = 0; j0 < 8; j0 += R) {
+        uint32_t nx[R][KW], cu[R][KW];
 #pragma unroll
-        for (int w = 0; w < KW; ++w) {
-          const uint32_t next = p.Vn[idx * KW + w], cur = p.Vc[idx * KW + w];
-          const uint32_t diff = next ^ cur;
-          p.F[idx * KW + w] = diff;  // PAPER.md:610 (unconditional)
-          if (diff) {
-            p.Vc[idx * KW + w] = next;
-            A |= diff;
-            pc += __popc(diff);
+        for (uint32_t r = 0; r < R; ++r) {
+          const uint64_t idx = (uint64_t)(j0 + r) * p.rho + s;
+          load_words<KW>(p.Vn, idx, nx[r]);
+          load_words<KW>(p.Vc, idx, cu[r]);
+        }
+#pragma unroll
+        for (uint32_t r = 0; r < R; ++r) {
+          const uint32_t j = j0 + r;
+          const uint64_t idx = (uint64_t)j * p.rho + s;
+          uint32_t diff[KW], pc = 0, any = 0;
+#pragma unroll
+          for (int w = 0; w < KW; ++w) {
+            diff[w] = nx[r][w] ^ cu[r][w];
+            any |= diff[w];
+            pc += __popc(diff[w]);
+          }
+          store_words<KW>(p.F, idx, diff);  // PAPER.md:610 (unconditional)
+          if (any) {
+            store_words<KW>(p.Vc, idx, nx[r]);
+            A |= any;
             if (perSource || p.levels) {
               const uint32_t u = s * 8u + j;
               const uint32_t uo = p.iperm ? __ldg(&p.iperm[u]) : u;
-              for (uint32_t d = diff; d; d &= d - 1) {
-                const uint32_t c = w * 32u + (__ffs(d) - 1);
-                if (perSource) atomicAdd(&sh.perSource[c], 1u);
-                if (p.levels) p.levels[(b0 + c) * (uint64_t)p.n + uo] = (int32_t)level;
-              }
+#pragma unroll
+              for (int w = 0; w < KW; ++w)
+                for (uint32_t d = diff[w]; d; d &= d - 1) {
+                  const uint32_t c = w * 32u + (__ffs(d) - 1);
+                  if (perSource) atomicAdd(&sh.perSource[c], 1u);
+                  if (p.levels) p.levels[(b0 + c) * (uint64_t)p.n + uo] = (int32_t)level;
+                }
             }
+            nnew += pc;
+            if (p.farT) p.farT[idx] += (unsigned long long)level * pc;  // Eq. 7: far[idx] += l * popc(diff)
+            if (p.reachT) p.reachT[idx] += pc;
           }
-        }
-        if (pc) {
-          nnew += pc;
-          if (p.farT) p.farT[idx] += (unsigned long long)level * pc;  // Eq. 7: far[idx] += l * popc(diff)
-          if (p.reachT) p.reachT[idx] += pc;
         }
       }
       if (A) {  // active in at least one BFS: enqueue all VSSs of the set
