@@ -53,6 +53,7 @@ struct BfsParams {
   float eta, gamma;
   // switch cost model, picoseconds per unit
   float cTdEdge, cTdVertex, cTdWord, cBuVertex, cBuScan, cBuWord;
+  float scanExp;  // exponent of nnz/mf in the estimate of neighbours examined per bottom-up vertex
 };
 
 struct MsParams {

@@ -780,7 +780,9 @@ __device__ __forceinline__ bool choose_bottom_up(const BfsParams& p, uint32_t le
   // Bottom-up examines, for every unvisited vertex, neighbours until the first one in the frontier: with a fraction
   // mf/nnz of all edge endpoints in the frontier that is about nnz/mf per vertex, and never more than its degree.
   const float fmf = (float)mf, fnu = (float)nu;
-  const float perVertex = fminf((float)p.nnz / fmaxf(fmf, 1.0f), fnu > 0.f ? (float)mu / fnu : 0.f);
+  // ... in a graph whose neighbours are met in random order.  After the degree sort the first neighbours are the hubs,
+  // which enter the frontier first: the traces fit (nnz/mf)^0.5 there (scanExp; 1 for unordered graphs).
+  const float perVertex = fminf(powf((float)p.nnz / fmaxf(fmf, 1.0f), p.scanExp), fnu > 0.f ? (float)mu / fnu : 0.f);
   const float costTd = p.cTdEdge * fmf + p.cTdVertex * (float)nf + p.cTdWord * (float)p.nSweepWords;
   const float costBu = p.cBuVertex * fnu + p.cBuScan * fnu * perVertex + p.cBuWord * (float)p.nSweepWords;
   return costBu * 10.0f < p.eta * costTd;
