@@ -32,7 +32,7 @@ static thread_local int g_lastCuda = 0;
 static constexpr uint32_t TRACE_CAP = 1u << 17;
 static constexpr double UDIV_THRESHOLD = 25000.0;
 // switch cost model defaults, picoseconds per unit
-static constexpr float COST_TD_EDGE = 20.0f, COST_TD_VERTEX = 40.0f, COST_TD_WORD = 30.0f;
+static constexpr float COST_TD_EDGE = 4.6f, COST_TD_NEW = 16.5f, COST_TD_VERTEX = 40.0f, COST_TD_WORD = 30.0f;
 static constexpr float COST_BU_VERTEX = 4.0f, COST_BU_SCAN = 4.5f, COST_BU_WORD = 20.0f;
 
 struct blest_graph {
@@ -477,7 +477,9 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
     float* dst[5] = {&p.cTdEdge, &p.cTdVertex, &p.cBuVertex, &p.cBuScan, &p.cBuWord};
     for (int k = 0; k < 5; ++k) *dst[k] = h->opt.reserved[1 + k] > 0 ? 0.01f * (float)h->opt.reserved[1 + k] : dflt[k];
     p.cTdWord = COST_TD_WORD;
+    p.cTdNew = COST_TD_NEW;
     p.scanExp = h->opt.reorder == 2 ? 0.5f : 1.0f;
+    p.hubFilter = h->opt.reorder == 2 ? 1 : 0;
   }
   p.switching = h->opt.switching;
   p.contraction = h->opt.contraction ? h->opt.contraction : 1;  // auto -> ALU (measured fastest)

@@ -9,7 +9,7 @@ constexpr uint32_t BIG_EDGES = 512;     // longer adjacency lists are deferred t
 constexpr uint32_t BIG_QUADS = 128;     // longer slice sets (in quads) are deferred to the balanced phase
 constexpr uint32_t CHUNK_EDGES = 256;   // balanced phase: edges per chunk entry
 constexpr uint32_t CHUNK_QUADS = 64;    // balanced phase: quads per chunk entry
-constexpr uint32_t WL_STAGE = 4096;     // per-CTA shared-memory staging of frontier word ids
+constexpr uint32_t WL_STAGE = 2048;     // per-CTA shared-memory staging of frontier word ids
 
 struct BfsParams {
   // graph (immutable during traversal)
@@ -52,7 +52,8 @@ struct BfsParams {
   uint32_t buMask;  // switching == 5: level l runs bottom-up iff bit min(l,31) is set
   float eta, gamma;
   // switch cost model, picoseconds per unit
-  float cTdEdge, cTdVertex, cTdWord, cBuVertex, cBuScan, cBuWord;
+  float cTdEdge, cTdNew, cTdVertex, cTdWord, cBuVertex, cBuScan, cBuWord;
+  int hubFilter;  // top-down marks of low-id vertices are de-duplicated per CTA (degree-sorted graphs)
   float scanExp;  // exponent of nnz/mf in the estimate of neighbours examined per bottom-up vertex
 };
 

@@ -20,6 +20,7 @@
 //             finalisation (#unvisited as in Eq. 6, plus degree sums), scaled by eta.
 //   output    levels_out is pre-filled with -1 ("infinity", reading R1) and the level of a vertex is
 //             written to levels_out[original id] at the moment it is finalised (A10 fused into A6 / Alg. 4).
+#include <cstddef>
 #include "bfs_kernels.cuh"
 
 namespace blest {
@@ -31,6 +32,7 @@ constexpr uint32_t NONE = 0xffffffffu;
 
 constexpr uint32_t BU_LIST = 512;   // per-warp list of unvisited vertices (sparse bottom-up groups)
 constexpr uint32_t BU_BATCH = 256;  // vertices per bottom-up batch: 8 per lane in flight
+constexpr uint32_t HUB_BITS = 1u << 17;  // top-down: marks of the first 2^17 vertices are de-duplicated per CTA in shared memory
 
 struct LazyShared {
   unsigned long long acc[6];
@@ -42,6 +44,7 @@ struct LazyShared {
   uint32_t buSlotTag[WARPS_PER_BLOCK][32];
   uint32_t buList[WARPS_PER_BLOCK][BU_LIST];
   uint32_t wl[WL_STAGE];
+  uint32_t hub[HUB_BITS / 32];  // top-down Stage 1: low-id vertices this CTA has already marked in this level
 };
 
 struct Counters {
@@ -121,15 +124,26 @@ __device__ __forceinline__ void prefetch_l2(const void* ptr) { asm volatile("pre
 // probeFn: also read F_next before the atomic.  It pays when a level has many more edges than unvisited vertices
 // (most marks would repeat an earlier one, and repeated atomics on a hot word serialise in L2); otherwise it is one
 // more scattered access per edge for nothing, so the level decides (mf > 4 nu).
+// hub: per-CTA shared bitmap over the first HUB_BITS vertex ids.  After the degree sort those are the hubs, the targets
+// of most edges: a shared-memory atomic drops the repeats before they cost a scattered probe and an L2 atomic on a hot
+// word (each CTA sends at most one mark per hub and level).
 struct Marks {
   const uint32_t* V;
   uint32_t* Fn;
   bool probeFn;
+  uint32_t* hub;
+  uint32_t hubLimit;  // HUB_BITS, or 0 = filter off (graphs that are not degree-sorted: low ids are no hubs there)
 };
 template <int U>
 __device__ __forceinline__ void mark_batch(const Marks& mk, const uint32_t (&v)[U], uint32_t valid) {
   const uint32_t* V = mk.V;
   uint32_t* Fn = mk.Fn;
+#pragma unroll
+  for (int j = 0; j < U; ++j)
+    if (((valid >> j) & 1u) && v[j] < mk.hubLimit) {
+      const uint32_t bit = 1u << (v[j] & 31u);
+      if (atomicOr(&mk.hub[v[j] >> 5], bit) & bit) valid &= ~(1u << j);
+    }
   uint32_t vw[U];
 #pragma unroll
   for (int j = 0; j < U; ++j) vw[j] = ((valid >> j) & 1u) ? V[v[j] >> 5] : FULL;
@@ -783,7 +797,12 @@ __device__ __forceinline__ bool choose_bottom_up(const BfsParams& p, uint32_t le
   // ... in a graph whose neighbours are met in random order.  After the degree sort the first neighbours are the hubs,
   // which enter the frontier first: the traces fit (nnz/mf)^0.5 there (scanExp; 1 for unordered graphs).
   const float perVertex = fminf(powf((float)p.nnz / fmaxf(fmf, 1.0f), p.scanExp), fnu > 0.f ? (float)mu / fnu : 0.f);
-  const float costTd = p.cTdEdge * fmf + p.cTdVertex * (float)nf + p.cTdWord * (float)p.nSweepWords;
+  // top-down: every edge out of the frontier is read and probed (cTdEdge); a vertex it discovers costs an atomic, a
+  // finalisation and a level write (cTdNew); mf edges thrown at nAct candidate vertices discover about
+  // nu (1 - exp(-mf / nAct)) of the nu unvisited ones (exact for the uniform graph, an over-estimate for skewed ones)
+  const float nAct = fmaxf((float)p.nSweepWords * 32.0f - (float)p.nIsoInSweep, 1.0f);
+  const float newEst = fnu * (1.0f - __expf(-fmf / nAct));
+  const float costTd = p.cTdEdge * fmf + p.cTdNew * newEst + p.cTdVertex * (float)nf + p.cTdWord * (float)p.nSweepWords;
   const float costBu = p.cBuVertex * fnu + p.cBuScan * fnu * perVertex + p.cBuWord * (float)p.nSweepWords;
   return costBu * 10.0f < p.eta * costTd;
 }
@@ -884,7 +903,11 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       if (leader) tStage1 = globaltimer();
     } else {
       if (level == 1) prefill_out();  // the stores drain while the (latency-bound) first expansion runs
-      const Marks mk{p.V, Fn, mf > 4ull * nu};
+      const Marks mk{p.V, Fn, p.hubFilter || mf > 4ull * nu, sh.hub, p.hubFilter ? HUB_BITS : 0u};
+      if (p.hubFilter) {
+        for (uint32_t i = threadIdx.x; i < HUB_BITS / 32; i += blockDim.x) sh.hub[i] = 0;
+        __syncthreads();
+      }
       td_phase_a<CONTR>(p, sh, p.WL[(level - 1) & 1u], wlCount, Fp, mk, ctrl, ci);
       grid_barrier(&ctrl->bar, epoch);
       if (level == 1 && leader) p.out[p.srcOrig] = 0;  // L[src] = 0 (after the fill: ordered by the barrier)
@@ -937,7 +960,9 @@ int coop_blocks(K kernel) {
 template <class K>
 cudaError_t coop_launch(K kernel, const BfsParams& p, int gridBlocks, cudaStream_t st) {
   void* args[] = {(void*)&p};
-  return cudaLaunchCooperativeKernel((const void*)kernel, dim3(gridBlocks), dim3(BLOCK_THREADS), args, sizeof(LazyShared), st);
+  // the hub bitmap is the last member: without the filter the launch leaves that shared memory to the L1
+  const size_t smem = p.hubFilter ? sizeof(LazyShared) : offsetof(LazyShared, hub);
+  return cudaLaunchCooperativeKernel((const void*)kernel, dim3(gridBlocks), dim3(BLOCK_THREADS), args, smem, st);
 }
 
 }  // namespace
