@@ -41,6 +41,7 @@ struct blest_graph {
   blest_options_t opt{};
   blest_info_t info{};
   bool hasPerm = false;
+  bool hubby = false;     // degree-sorted AND scale-free-like: the first 1 % of the vertices own >= 20 % of the edge endpoints
   bool hostOnly = false;  // blest_preprocess_host: no device arrays, traversal calls are refused
   HostBvss hb;            // kept only when hostOnly
   HostCsr hcsr;           // kept only when hostOnly
@@ -291,6 +292,10 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
       for (uint32_t w = 0; w < g->nSweepWords; ++w) iso += (uint32_t)__builtin_popcount(g->isoBits[w]);
       g->nIsoInSweep = iso;
     }
+    // scale-free-like test in the spirit of PAPER.md:199 (fn. 2: the top 1 % of the vertices hold a large share of the
+    // degree); only meaningful after the degree sort, where the top vertices are the first ones
+    g->hubby = opt.reorder == 2 && g->nnz > 0 &&
+               (double)gcsr->rowptr[std::max<uint32_t>(g->n / 100u, 1u)] >= 0.20 * (double)g->nnz;
     g->realPtrs.swap(b.realPtrs);
     g->virtualToReal.swap(b.virtualToReal);
     g->opt = opt;
@@ -478,8 +483,8 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
     for (int k = 0; k < 5; ++k) *dst[k] = h->opt.reserved[1 + k] > 0 ? 0.01f * (float)h->opt.reserved[1 + k] : dflt[k];
     p.cTdWord = COST_TD_WORD;
     p.cTdNew = COST_TD_NEW;
-    p.scanExp = h->opt.reorder == 2 ? 0.5f : 1.0f;
-    p.hubFilter = h->opt.reorder == 2 ? 1 : 0;
+    p.scanExp = h->hubby ? 0.5f : 1.0f;
+    p.hubFilter = h->hubby ? 1 : 0;
   }
   p.switching = h->opt.switching;
   p.contraction = h->opt.contraction ? h->opt.contraction : 1;  // auto -> ALU (measured fastest)
@@ -498,7 +503,12 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
     // so that those 4-byte writes merge there instead of each costing DRAM a sector.  Measured on C4: -5..10 % per BFS.
     const size_t bytes = (size_t)h->n * 4;
     static const bool envOff = getenv("BLEST_PERSIST") && atoi(getenv("BLEST_PERSIST")) == 0;
-    const bool usePersist = !envOff && h->hasPerm && g_persistMax() > 0 && bytes <= (size_t)g_windowMax();
+    const bool usePersist = !envOff && h->hasPerm && bytes <= (size_t)g_persistMax() && bytes <= (size_t)g_windowMax();
+    // reordered graph: levels scattered straight into levels_out when L2 can hold it, else internal array + gather pass
+    p.gather = h->hasPerm && !usePersist;
+    p.lvl = p.gather ? h->dL : p.out;
+    p.ipermW = (h->hasPerm && !p.gather) ? h->dIperm : nullptr;
+    p.srcLvl = p.gather ? p.src : src;
     set_persisting_l2(usePersist ? (size_t)g_persistMax() : 0);
     if (usePersist) {
       cudaStreamAttrValue av{};

@@ -41,6 +41,11 @@ struct BfsParams {
   int32_t* stamp;  // last level at which a slice set was enqueued
   // levels
   int32_t* out;    // levels in ORIGINAL ids (device)
+  int32_t* lvl;    // lazy kernel: where a finalised vertex's level is written: out (index = original id) or, with
+                   // `gather`, the internal-id array L
+  const uint32_t* ipermW;  // lazy kernel: iperm when lvl is indexed by original ids of a reordered graph, else nullptr
+  uint32_t srcLvl;         // index of the source in lvl
+  int gather;              // lazy kernel: final pass out[v] = lvl[perm[v]]
   int32_t* L;      // levels in internal ids (== out when there is no reordering)
   Ctrl* ctrl;
   blest_level_trace_t* trace;

@@ -19,7 +19,9 @@
 //   switch    start of each level: estimated cost of the two directions from the counters of the previous
 //             finalisation (#unvisited as in Eq. 6, plus degree sums), scaled by eta.
 //   output    levels_out is pre-filled with -1 ("infinity", reading R1) and the level of a vertex is
-//             written to levels_out[original id] at the moment it is finalised (A10 fused into A6 / Alg. 4).
+//             written to levels_out[original id] at the moment it is finalised (A10 fused into A6 / Alg. 4) -- when
+//             the array fits the persisting-L2 window; otherwise levels go to an internal-id array and a final
+//             gather pass moves them (scattered writes that miss L2 cost DRAM a read-modify-write each).
 #include <cstddef>
 #include "bfs_kernels.cuh"
 
@@ -430,14 +432,14 @@ __device__ __forceinline__ void write_levels_dense(const BfsParams& p, uint32_t 
     }
     uint32_t o[8], dg[8];
 #pragma unroll
-    for (int q = 0; q < 8; ++q) o[q] = ((on >> q) & 1u) ? (p.iperm ? __ldg(&p.iperm[u[q]]) : u[q]) : 0u;
+    for (int q = 0; q < 8; ++q) o[q] = ((on >> q) & 1u) ? (p.ipermW ? __ldg(&p.ipermW[u[q]]) : u[q]) : 0u;
 #pragma unroll
     for (int q = 0; q < 8; ++q) dg[q] = ((on >> q) & 1u) ? __ldg(&p.deg[u[q]]) : 0u;
 #pragma unroll
     for (int q = 0; q < 8; ++q) c.mf += dg[q];
 #pragma unroll
     for (int q = 0; q < 8; ++q)
-      if ((on >> q) & 1u) p.out[o[q]] = level;
+      if ((on >> q) & 1u) p.lvl[o[q]] = level;
   }
 }
 // Same for a lane's own sparse word (a few bits): four vertices in flight.
@@ -455,7 +457,7 @@ __device__ __forceinline__ void write_levels_sparse(const BfsParams& p, uint32_t
       }
     }
 #pragma unroll
-    for (int q = 0; q < 4; ++q) o[q] = on[q] ? (p.iperm ? __ldg(&p.iperm[u[q]]) : u[q]) : 0u;
+    for (int q = 0; q < 4; ++q) o[q] = on[q] ? (p.ipermW ? __ldg(&p.ipermW[u[q]]) : u[q]) : 0u;
     uint32_t dg[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) dg[q] = on[q] ? __ldg(&p.deg[u[q]]) : 0u;
@@ -463,7 +465,7 @@ __device__ __forceinline__ void write_levels_sparse(const BfsParams& p, uint32_t
     for (int q = 0; q < 4; ++q) c.mf += dg[q];
 #pragma unroll
     for (int q = 0; q < 4; ++q)
-      if (on[q]) p.out[o[q]] = level;
+      if (on[q]) p.lvl[o[q]] = level;
   }
 }
 
@@ -673,7 +675,7 @@ __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uin
     const uint32_t found = bu_resolve<false>(p, Fp, fshare, slotU, slotTag, lane, u, c, list, listCount);
     uint32_t o[8], dg[8];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) o[k] = ((found >> k) & 1u) ? (p.iperm ? __ldg(&p.iperm[u[k] & ~CSR_STAGE]) : (u[k] & ~CSR_STAGE)) : 0u;
+    for (int k = 0; k < 8; ++k) o[k] = ((found >> k) & 1u) ? (p.ipermW ? __ldg(&p.ipermW[u[k] & ~CSR_STAGE]) : (u[k] & ~CSR_STAGE)) : 0u;
 #pragma unroll
     for (int k = 0; k < 8; ++k) dg[k] = ((found >> k) & 1u) ? __ldg(&p.deg[u[k] & ~CSR_STAGE]) : 0u;
     {
@@ -689,7 +691,7 @@ __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uin
       oldF[k] = 1u;
       if ((found >> k) & 1u) {
         const uint32_t uu = u[k] & ~CSR_STAGE, bit = 1u << (uu & 31u);
-        p.out[o[k]] = (int32_t)level;
+        p.lvl[o[k]] = (int32_t)level;
         atomicOr(&p.V[uu >> 5], bit);
         oldF[k] = atomicOr(&Fn[uu >> 5], bit);
       }
@@ -731,7 +733,7 @@ __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uin
         const uint32_t found = bu_resolve<true>(p, Fp, fshare, slotU, slotTag, lane, u, c, list, listCount);
         uint32_t o[8], dg[8];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) o[k] = ((found >> k) & 1u) ? (p.iperm ? __ldg(&p.iperm[u[k]]) : u[k]) : 0u;
+        for (int k = 0; k < 8; ++k) o[k] = ((found >> k) & 1u) ? (p.ipermW ? __ldg(&p.ipermW[u[k]]) : u[k]) : 0u;
 #pragma unroll
         for (int k = 0; k < 8; ++k) dg[k] = ((found >> k) & 1u) ? __ldg(&p.deg[u[k]]) : 0u;
         {
@@ -742,7 +744,7 @@ __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uin
         }
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-          if ((found >> k) & 1u) p.out[o[k]] = (int32_t)level;  // lane = bit: coalesced when there is no reordering
+          if ((found >> k) & 1u) p.lvl[o[k]] = (int32_t)level;  // lane = bit: coalesced when there is no reordering
           const uint32_t fmk = __ballot_sync(FULL, (found >> k) & 1u);
           if (lane == 8u * sub + k) fmw = fmk;
         }
@@ -845,7 +847,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
   // warps busy and writes no level; the barrier after it orders the fill before every level write.
   auto prefill_out = [&]() {
   {
-      uint32_t* o = reinterpret_cast<uint32_t*>(p.out);
+      uint32_t* o = reinterpret_cast<uint32_t*>(p.lvl);
       const uint64_t head = min((uint64_t)p.n, (uint64_t)((16u - ((uintptr_t)o & 15u)) & 15u) >> 2);
       const uint64_t n4 = ((uint64_t)p.n - head) >> 2;
       uint4* o4 = reinterpret_cast<uint4*>(o + head);
@@ -896,7 +898,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       if (level == 1) {  // (scripted direction only)
         prefill_out();
         grid_barrier(&ctrl->bar, epoch);
-        if (leader) p.out[p.srcOrig] = 0;
+        if (leader) p.lvl[p.srcLvl] = 0;
       }
       bu_level(p, sh, level, Fp, Fn, Fs, p.WL[level & 1u], ctrl, ci, nu);
       grid_barrier(&ctrl->bar, epoch);
@@ -910,7 +912,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       }
       td_phase_a<CONTR>(p, sh, p.WL[(level - 1) & 1u], wlCount, Fp, mk, ctrl, ci);
       grid_barrier(&ctrl->bar, epoch);
-      if (level == 1 && leader) p.out[p.srcOrig] = 0;  // L[src] = 0 (after the fill: ordered by the barrier)
+      if (level == 1 && leader) p.lvl[p.srcLvl] = 0;  // L[src] = 0 (after the fill: ordered by the barrier)
       if (threadIdx.x == 0) sh.ctl[0] = ld_volatile(&ctrl->qc[ci]);
       __syncthreads();
       const uint32_t nChunks = (uint32_t)sh.ctl[0];
@@ -940,6 +942,23 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     }
   }
   if (leader) ctrl->nlevels = level - 1;
+
+  // A10 as a separate pass (p.gather): the levels were written in internal ids (coalesced, no iperm read) and go to
+  // original ids here.  Used when levels_out is too big to be held in L2 by the persisting window: scattered 4-byte
+  // writes then cost DRAM a read-modify-write each (measured: 100 ps per vertex on C3 + RCM against 10 ps for this pass).
+  if (p.gather) {
+    for (uint64_t v0 = gtid * 4; v0 < p.n; v0 += nth * 4) {
+      uint32_t pv[4];
+      int32_t lv[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) pv[j] = v0 + j < p.n ? __ldcs(&p.perm[v0 + j]) : 0u;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) lv[j] = v0 + j < p.n ? p.lvl[pv[j]] : 0;
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+        if (v0 + j < p.n) p.out[v0 + j] = lv[j];
+    }
+  }
 }
 
 __global__ void isolated_source_kernel(int32_t* out, uint32_t n, uint32_t src) {
