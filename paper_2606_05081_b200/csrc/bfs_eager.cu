@@ -58,23 +58,19 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_eager_kernel(const __gri
     const uint32_t nent = seg_entries(0, nq);
     if (nent <= p.qcap) {
       for (uint32_t i = lane; i < nent; i += 32) write_entry(p.Q[1], 0, 0, a, nq, s0, i);
-      if (lane == 0) ctrl->qc[1] = nent;
+      if (lane == 0) ctrl->tail = nent;
     } else if (lane == 0) atomicOr(&ctrl->error, 1u);
   }
-  grid_barrier(&ctrl->bar, epoch);
+  // The queue tail is ONE monotone counter: the entries of level l+1 take positions [tEnd_l, tEnd_{l+1}) and live in
+  // Q[(l+1) & 1] at (position - tEnd_l).  The barrier hands every CTA the tail, so no queue length is read or reset.
+  uint32_t tStart = 0, tEnd = grid_barrier_tail(&ctrl->bar, epoch, &sh.qcount);
 
   uint32_t level = 1;
   for (;; ++level) {
-    // one thread per CTA reads the queue length (every warp reading it would queue on one L2 slice)
-    if (threadIdx.x == 0) sh.qcount = ld_volatile(&ctrl->qc[level % 3u]);
-    __syncthreads();
-    const uint32_t qcount = sh.qcount;
-    __syncthreads();
+    const uint32_t qcount = tEnd - tStart;
     if (qcount == 0) break;
     const uint2* Qc = p.Q[level & 1u];
     uint2* Qn = p.Q[(level + 1) & 1u];
-    unsigned int* qcn = &ctrl->qc[(level + 1) % 3u];
-    if (blockIdx.x == 0 && threadIdx.x == 0) ctrl->qc[(level + 2) % 3u] = 0;
     BigSeg* bigList = sh.bigList[warp];
     uint32_t* bigCnt = &sh.bigCnt[warp];
     for (uint32_t i = gwarp; i < qcount; i += nwarps) {
@@ -123,12 +119,18 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_eager_kernel(const __gri
         }
       }
       bool ok;
-      uint32_t pos = warp_reserve(qcn, cnt, lane, p.qcap, &ctrl->error, ok);
+      uint32_t pos = warp_reserve(&ctrl->tail, cnt, lane, 0xFFFFFFFFu, &ctrl->error, ok) - tEnd;
+      {  // capacity of the next level's queue (the tail itself never wraps: every VSS is enqueued <= 8 times per call)
+        const uint32_t tot = __reduce_add_sync(0xffffffffu, cnt), first = __shfl_sync(0xffffffffu, pos, 0);
+        ok = tot == 0u || (uint64_t)first + tot <= p.qcap;
+        if (!ok && lane == 0) atomicOr(&ctrl->error, 1u);
+      }
       if (ok)
         for (uint32_t k = 0; k < nseg; ++k) emit_segment(Qn, pos, 0, segA[k], segN[k], segS[k], bigList, bigCnt);
       flush_big_segments(Qn, bigList, bigCnt, lane);
     }
-    grid_barrier(&ctrl->bar, epoch);
+    tStart = tEnd;
+    tEnd = grid_barrier_tail(&ctrl->bar, epoch, &sh.qcount);
     if (blockIdx.x == 0 && threadIdx.x == 0 && p.trace && level - 1 < p.traceCap) {
       blest_level_trace_t r;
       r.level = level;

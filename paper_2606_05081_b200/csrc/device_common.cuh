@@ -18,9 +18,10 @@ constexpr uint32_t BIG_CAP = 16;       // per-warp capacity of the cooperative-e
 // Control block in global memory, zeroed by the host before every launch.
 struct Ctrl {
   unsigned int bar;    // monotone grid-barrier arrival counter
+  unsigned int tail;   // eager kernel: monotone work-queue tail; shares an aligned 8-byte word with `bar`, so the
+                       // barrier's spin load returns both (one round trip less per level)
   unsigned int error;  // bit 0: work-queue overflow
   unsigned int nlevels;
-  unsigned int pad0;
   unsigned int qc[4];               // work-queue entry counters (rotating)
   unsigned long long qbytes[4];     // graph bytes covered by the work of each level (rotating)
   unsigned long long unvisited[4];  // per level (rotating)
@@ -53,6 +54,24 @@ __device__ __forceinline__ void grid_barrier(unsigned int* bar, unsigned int& ep
     } while (v < target);
   }
   __syncthreads();
+}
+
+// Same barrier on the {bar, tail} word: returns the queue tail as it stands once every CTA has arrived (each CTA's
+// appends precede its arrival, so the value is final).  `slot` is a shared-memory word for the broadcast.
+__device__ __forceinline__ unsigned int grid_barrier_tail(unsigned int* bar, unsigned int& epoch, unsigned int* slot) {
+  __syncthreads();
+  ++epoch;
+  if (threadIdx.x == 0) {
+    const unsigned int target = epoch * gridDim.x;
+    asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(bar) : "memory");
+    unsigned long long v;
+    do {
+      asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(bar) : "memory");
+    } while ((unsigned int)v < target);
+    *slot = (unsigned int)(v >> 32);
+  }
+  __syncthreads();
+  return *slot;
 }
 
 template <class T>
