@@ -34,6 +34,7 @@ constexpr uint32_t NONE = 0xffffffffu;
 
 constexpr uint32_t BU_LIST = 512;   // per-warp list of unvisited vertices (sparse bottom-up groups)
 constexpr uint32_t BU_BATCH = 256;  // vertices per bottom-up batch: 8 per lane in flight
+constexpr uint32_t DLIST_CAP = 1024;  // finalisation: dense words a CTA pools before its warps share them
 constexpr uint32_t HUB_BITS = 1u << 17;  // top-down: marks of the first 2^17 vertices are de-duplicated per CTA in shared memory
 
 struct LazyShared {
@@ -46,6 +47,8 @@ struct LazyShared {
   uint32_t buSlotTag[WARPS_PER_BLOCK][32];
   uint32_t buList[WARPS_PER_BLOCK][BU_LIST];
   uint32_t wl[WL_STAGE];
+  uint32_t dcount, dvalid;      // finalisation: dense words shared by the CTA's warps
+  uint2 dlist[DLIST_CAP];       // (word id, new-frontier bits)
   uint32_t hub[HUB_BITS / 32];  // top-down Stage 1: low-id vertices this CTA has already marked in this level
 };
 
@@ -469,13 +472,48 @@ __device__ __forceinline__ void write_levels_sparse(const BfsParams& p, uint32_t
   }
 }
 
+// Levels of up to eight (word, bits) entries of the CTA's dense list at a time (lane = bit).
+__device__ __forceinline__ void write_levels_list(const BfsParams& p, const uint2* ent, uint32_t cnt, int32_t level,
+                                                  uint32_t lane, Counters& c) {
+  uint32_t u[8], on = 0;
+#pragma unroll
+  for (int q = 0; q < 8; ++q) {
+    u[q] = 0;
+    if ((uint32_t)q < cnt) {
+      const uint2 e = ent[q];  // same address in all lanes: a broadcast
+      on |= ((e.y >> lane) & 1u) << q;
+      u[q] = e.x * 32u + lane;
+    }
+  }
+  uint32_t o[8], dg[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) o[q] = ((on >> q) & 1u) ? (p.ipermW ? __ldg(&p.ipermW[u[q]]) : u[q]) : 0u;
+#pragma unroll
+  for (int q = 0; q < 8; ++q) dg[q] = ((on >> q) & 1u) ? __ldg(&p.deg[u[q]]) : 0u;
+  uint32_t sum = 0;
+#pragma unroll
+  for (int q = 0; q < 8; ++q) sum += dg[q];
+  c.mf += sum;
+#pragma unroll
+  for (int q = 0; q < 8; ++q)
+    if ((on >> q) & 1u) p.lvl[o[q]] = level;
+}
+
 // Stage 2 after a top-down Stage 1: frontier finalisation (readings R9/R10).
 __device__ __forceinline__ void td_finalize(const BfsParams& p, LazyShared& sh, uint32_t level, uint32_t* Fn, uint32_t* Fs,
                                             uint32_t* WLn, Ctrl* ctrl, uint32_t ci) {
-  const uint32_t lane = threadIdx.x & 31;
-  const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
+  const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + warp, nwarps = gridDim.x * WARPS_PER_BLOCK;
+  // Consecutive 32-word batches go to warps of DIFFERENT CTAs (odd multiplier, coprime to the warp count), and the
+  // dense words a CTA finds are pooled and shared by its 32 warps: after a degree sort the discoveries of an early
+  // level sit in a few thousand consecutive words, which would otherwise be 1 024 level writes each for ~170 warps
+  // (4 x 4.5 us of dependent rounds) while 4 500 warps wait.
+  const uint32_t mult = (nwarps % 149u) ? 149u : 1u;
+  const uint32_t first = (uint32_t)(((uint64_t)gwarp * mult) % nwarps);
+  if (threadIdx.x == 0) { sh.dcount = 0; sh.dvalid = 0; }
+  __syncthreads();
   Counters c;
-  for (uint32_t wb = gwarp * 32u; wb < p.nSweepWords; wb += nwarps * 32u) {
+  for (uint32_t wb = first * 32u; wb < p.nSweepWords; wb += nwarps * 32u) {
     const uint32_t t = wb + lane;
     uint32_t fm = 0;
     if (t < p.nSweepWords) {
@@ -491,10 +529,30 @@ __device__ __forceinline__ void td_finalize(const BfsParams& p, LazyShared& sh, 
     // next level's work list (PAPER.md:420-440 enqueues the VSSs of every newly active slice set; here the non-zero
     // frontier word is the unit, expanded at consumption time)
     wl_append(sh, WLn, &ctrl->wlc[ci], t, fm != 0, lane);
-    // level once per discovered vertex: dense words by the warp (lane = bit), sparse ones by their lane
+    // level once per discovered vertex: sparse words by their own lane, dense ones pooled per CTA
     const bool dense = __popc(fm) > 6;
-    write_levels_dense(p, wb, fm, __ballot_sync(FULL, dense), (int32_t)level, lane, c);
+    const uint32_t dmask = __ballot_sync(FULL, dense);
+    if (dmask) {
+      uint32_t base = 0;
+      const uint32_t nd = (uint32_t)__popc(dmask);
+      if (lane == 0) {
+        base = atomicAdd(&sh.dcount, nd);
+        if (base + nd <= DLIST_CAP) atomicMax(&sh.dvalid, base + nd);
+      }
+      base = __shfl_sync(FULL, base, 0);
+      if (base + nd <= DLIST_CAP) {
+        if (dense) sh.dlist[base + __popc(dmask & ((1u << lane) - 1u))] = make_uint2(t, fm);
+      } else {
+        write_levels_dense(p, wb, fm, dmask, (int32_t)level, lane, c);  // pool full: the owner does them itself
+      }
+    }
     if (!dense) write_levels_sparse(p, t, fm, (int32_t)level, c);
+  }
+  __syncthreads();
+  {
+    const uint32_t nd = sh.dvalid;  // entries [0, nd) are valid: reservations are monotone, the first failure ends them
+    for (uint32_t e = warp * 8u; e < nd; e += WARPS_PER_BLOCK * 8u)
+      write_levels_list(p, &sh.dlist[e], min(8u, nd - e), (int32_t)level, lane, c);
   }
   wl_flush(sh, WLn, &ctrl->wlc[ci]);
   block_accumulate(sh, c, ctrl, ci);
