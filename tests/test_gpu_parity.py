@@ -273,3 +273,28 @@ def test_bad_arguments(blest, torch_cuda):
             g.msbfs(np.array([n], np.uint32), torch.empty((1, n), dtype=torch.int32, device="cuda"))
         with pytest.raises(blest.BlestError):
             g.closeness(torch.empty(3, dtype=torch.float64, device="cuda"), srcs=np.array([0, 1, n + 5], np.uint32))
+
+
+def test_gather_handoff_path_in_subprocess(blest, torch_cuda):
+    """Reordered graphs whose levels_out does not fit the persisting-L2 window use internal-id levels + a final gather pass
+    (C3-sized arrays).  BLEST_PERSIST=0 forces that path on small graphs; the variable is read once per process."""
+    import os
+    import subprocess
+    import sys
+
+    code = (
+        "import numpy as np, torch, graphgen as gg, oracle, paper_2606_05081_b200 as blest\n"
+        "for maker in (lambda: gg.rmat(12, 16, 9), lambda: gg.disjoint_union(gg.path(9), gg.empty(5), gg.complete(6)), lambda: gg.gnm(1003, 2500, 7)):\n"
+        "    n, rp, ci = maker()\n"
+        "    for reorder in ('degree', 'rcm'):\n"
+        "        with blest.Graph(n, rp, ci, kernel='lazy', reorder=reorder) as g:\n"
+        "            out = torch.full((n,), 7, dtype=torch.int32, device='cuda')\n"
+        "            for s in (0, n // 2, n - 1):\n"
+        "                g.bfs(s, out)\n"
+        "                assert np.array_equal(out.cpu().numpy(), oracle.bfs(n, rp, ci, s)), (reorder, s)\n"
+        "print('gather ok')\n"
+    )
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, BLEST_PERSIST="0", PYTHONPATH=root)
+    r = subprocess.run([sys.executable, "-c", code], env=env, cwd=root, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "gather ok" in r.stdout, r.stderr[-2000:]
