@@ -20,7 +20,7 @@ struct MsShared {
   BigSeg bigList[WARPS_PER_BLOCK][BIG_CAP];
   uint32_t bigCnt[WARPS_PER_BLOCK];
   unsigned long long acc;
-  unsigned long long ctl[2];  // control words of the level, read by one thread and broadcast
+  unsigned int tailSlot;  // broadcast slot of grid_barrier_tail
   uint32_t perSource[256];
   uint32_t fset[WARPS_PER_BLOCK][8 * 8];  // per warp: the kappa-bit frontier words of the current set's 8 columns
 };
@@ -125,12 +125,11 @@ __device__ __forceinline__ void ms_stage1(const MsParams& p, MsShared& sh, const
 
 template <int KW>
 __device__ __forceinline__ void ms_stage2(const MsParams& p, MsShared& sh, uint32_t level, uint64_t b0, uint32_t nb,
-                                          uint2* Qn, unsigned int* qcn, uint32_t par) {
+                                          uint2* Qn, uint32_t tBase) {
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + warp, nwarps = gridDim.x * WARPS_PER_BLOCK;
   BigSeg* bigList = sh.bigList[warp];
   uint32_t* bigCnt = &sh.bigCnt[warp];
-  unsigned long long nnew = 0;
   const bool perSource = (p.farS != nullptr) || (p.reachS != nullptr);
   for (uint64_t sb = (uint64_t)gwarp * 32; sb < p.Ns; sb += (uint64_t)nwarps * 32) {
     const uint32_t s = (uint32_t)sb + lane;  // consecutive threads -> consecutive slice sets
@@ -174,7 +173,6 @@ __device__ __forceinline__ void ms_stage2(const MsParams& p, MsShared& sh, uint3
                   if (p.levels) p.levels[(b0 + c) * (uint64_t)p.n + uo] = (int32_t)level;
                 }
             }
-            nnew += pc;
             if (p.farT) p.farT[idx] += (unsigned long long)level * pc;  // Eq. 7: far[idx] += l * popc(diff)
             if (p.reachT) p.reachT[idx] += pc;
           }
@@ -187,18 +185,18 @@ __device__ __forceinline__ void ms_stage2(const MsParams& p, MsShared& sh, uint3
       }
     }
     bool ok;
-    uint32_t pos = warp_reserve(qcn, cnt, lane, p.qcap, &p.ctrl->error, ok);
+    // one monotone queue tail for the whole launch (it shares the barrier's word, see grid_barrier_tail); positions
+    // are relative to the tail at the start of this sweep; modular arithmetic makes a 32-bit wrap harmless
+    uint32_t pos = warp_reserve(&p.ctrl->tail, cnt, lane, 0xFFFFFFFFu, &p.ctrl->error, ok) - tBase;
+    {
+      const uint32_t tot = __reduce_add_sync(0xffffffffu, cnt), first = __shfl_sync(0xffffffffu, pos, 0);
+      ok = tot == 0u || (uint64_t)first + tot <= p.qcap;
+      if (!ok && lane == 0) atomicOr(&p.ctrl->error, 1u);
+    }
     if (cnt && ok) emit_segment(Qn, pos, 0, a, nq, s, bigList, bigCnt);
     flush_big_segments(Qn, bigList, bigCnt, lane);
   }
-#pragma unroll
-  for (int d = 16; d > 0; d >>= 1) nnew += __shfl_down_sync(0xffffffffu, nnew, d);
-  if (lane == 0 && nnew) atomicAdd(&sh.acc, nnew);
   __syncthreads();
-  if (threadIdx.x == 0) {
-    if (sh.acc) atomicAdd(&p.ctrl->newcount[par], sh.acc);
-    sh.acc = 0;
-  }
   if (perSource && threadIdx.x < nb) {
     const uint32_t k = sh.perSource[threadIdx.x];
     if (k) {
@@ -224,6 +222,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_co
   __syncthreads();
   const uint64_t stateWords = (uint64_t)p.rho * 8u * KW;
 
+  uint32_t tStart = 0, tEnd = 0;  // queue tail before / after the sweep that filled the current level's queue
   for (uint64_t b0 = 0; b0 < p.nsrcs; b0 += KAPPA) {
     const uint32_t nb = (uint32_t)min((uint64_t)KAPPA, p.nsrcs - b0);
     // init(srcs, ...) (reading R16): visited words cleared, bit c of source c set, its set marked dirty
@@ -244,28 +243,24 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_co
     }
     grid_barrier(&ctrl->bar, epoch);
     // level 0 = the finalisation sweep over the sources themselves (far += 0, reach += 1, level 0, enqueue their sets)
-    ms_stage2<KW>(p, sh, 0, b0, nb, p.Q[1], &ctrl->qc[1], 0);
-    grid_barrier(&ctrl->bar, epoch);
+    ms_stage2<KW>(p, sh, 0, b0, nb, p.Q[1], tEnd);
+    {
+      const uint32_t t = grid_barrier_tail(&ctrl->bar, epoch, &sh.tailSlot);
+      tStart = tEnd;
+      tEnd = t;
+    }
     for (uint32_t level = 1;; ++level) {
-      const uint32_t pp = (level - 1) & 1u, par = level & 1u;
-      // one thread per CTA reads the control words (every warp reading them would queue on one L2 slice)
-      if (threadIdx.x == 0) {
-        sh.ctl[0] = ld_volatile(&ctrl->newcount[pp]);
-        sh.ctl[1] = ld_volatile(&ctrl->qc[par]);
-      }
-      __syncthreads();
-      const unsigned long long nnewPrev = sh.ctl[0];
-      const uint32_t qcount = (uint32_t)sh.ctl[1];
-      __syncthreads();
-      if (nnewPrev == 0) break;
+      const uint32_t par = level & 1u;
+      // a level whose sweep enqueued nothing discovered nothing (every discovered vertex has a neighbour, so its slice
+      // set has slices): the queue length the barrier returned is the termination test
+      const uint32_t qcount = tEnd - tStart;
+      if (qcount == 0) break;
       ms_stage1<KW>(p, sh, p.Q[par], qcount);
       grid_barrier(&ctrl->bar, epoch);
-      if (blockIdx.x == 0 && threadIdx.x == 0) {
-        ctrl->qc[par] = 0;
-        ctrl->newcount[pp] = 0;
-      }
-      ms_stage2<KW>(p, sh, level, b0, nb, p.Q[par ^ 1u], &ctrl->qc[par ^ 1u], par);
-      grid_barrier(&ctrl->bar, epoch);
+      ms_stage2<KW>(p, sh, level, b0, nb, p.Q[par ^ 1u], tEnd);
+      const uint32_t t = grid_barrier_tail(&ctrl->bar, epoch, &sh.tailSlot);
+      tStart = tEnd;
+      tEnd = t;
     }
   }
 }
