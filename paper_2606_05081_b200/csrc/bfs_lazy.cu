@@ -889,7 +889,20 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     p.F[1][i] = 0;
     p.F[2][i] = 0;
   }
-  const uint32_t srcDeg = __ldg(&p.rowptr[p.src + 1]) - __ldg(&p.rowptr[p.src]);
+  // levels = -1 everywhere (reading R1), before any level is written
+  {
+    uint32_t* o = reinterpret_cast<uint32_t*>(p.lvl);
+    const uint64_t head = min((uint64_t)p.n, (uint64_t)((16u - ((uintptr_t)o & 15u)) & 15u) >> 2);
+    const uint64_t n4 = ((uint64_t)p.n - head) >> 2;
+    uint4* o4 = reinterpret_cast<uint4*>(o + head);
+    const uint4 m1 = make_uint4(NONE, NONE, NONE, NONE);
+    for (uint64_t i = gtid; i < n4; i += nth) o4[i] = m1;
+    const uint64_t tail0 = head + (n4 << 2);
+    if (gtid < head) o[gtid] = NONE;
+    if (gtid < (uint64_t)p.n - tail0) o[tail0 + gtid] = NONE;
+  }
+  const uint32_t srcRow = __ldg(&p.rowptr[p.src]);
+  const uint32_t srcDeg = __ldg(&p.rowptr[p.src + 1]) - srcRow;
   if (leader) {
     // level 0: the source itself (frontier = {src})
     p.WL[0][0] = srcWord;
@@ -899,23 +912,11 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     ctrl->unvisited[0] = (unsigned long long)min((uint64_t)p.n, (uint64_t)nSW * 32u) - 1u - p.nIsoInSweep;
   }
   grid_barrier(&ctrl->bar, epoch);
-  if (leader) ctrl->tInit = globaltimer() - ctrl->t0;
+  if (leader) {
+    ctrl->tInit = globaltimer() - ctrl->t0;
+    p.lvl[p.srcLvl] = 0;  // L[src] = 0 (after the fill: ordered by the barrier)
+  }
 
-  // levels_out = -1 everywhere (reading R1).  Runs next to level 1's Stage 1, which keeps only a few
-  // warps busy and writes no level; the barrier after it orders the fill before every level write.
-  auto prefill_out = [&]() {
-  {
-      uint32_t* o = reinterpret_cast<uint32_t*>(p.lvl);
-      const uint64_t head = min((uint64_t)p.n, (uint64_t)((16u - ((uintptr_t)o & 15u)) & 15u) >> 2);
-      const uint64_t n4 = ((uint64_t)p.n - head) >> 2;
-      uint4* o4 = reinterpret_cast<uint4*>(o + head);
-      const uint4 m1 = make_uint4(NONE, NONE, NONE, NONE);
-      for (uint64_t i = gtid; i < n4; i += nth) o4[i] = m1;
-      const uint64_t tail0 = head + (n4 << 2);
-      if (gtid < head) o[gtid] = NONE;
-      if (gtid < (uint64_t)p.n - tail0) o[tail0 + gtid] = NONE;
-    }
-  };
   unsigned long long degVisited = 0;  // sum of degrees of all visited vertices
   uint32_t level = 1;
   for (;; ++level) {
@@ -952,17 +953,44 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       ctrl->qc[cn] = 0;
     }
     unsigned long long tStage1 = 0;
-    if (bottomUp) {
-      if (level == 1) {  // (scripted direction only)
-        prefill_out();
-        grid_barrier(&ctrl->bar, epoch);
-        if (leader) p.lvl[p.srcLvl] = 0;
+    if (level == 1 && !bottomUp && p.switching == 0) {
+      // Level 1 needs no probe, no filter and no sweep: the neighbours of the source are distinct and all unvisited, so
+      // each edge of the source finalises its target on the spot (one phase, one barrier instead of two and a sweep).
+      Counters c;
+      const uint32_t lane = threadIdx.x & 31;
+      const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
+      for (uint32_t base = gwarp * 32u; base < srcDeg; base += nwarps * 32u) {
+        const bool active = base + lane < srcDeg;
+        const uint32_t v = active ? __ldcs(p.colidx + srcRow + base + lane) : 0u;
+        const uint32_t bit = 1u << (v & 31u);
+        uint32_t old = FULL;
+        if (active) old = atomicOr(&Fn[v >> 5], bit);
+        const bool disc = active && !(old & bit);  // (a duplicated CSR entry is not discovered twice)
+        uint32_t o = 0, dg = 0;
+        if (disc) {
+          o = p.ipermW ? __ldg(&p.ipermW[v]) : v;
+          dg = __ldg(&p.deg[v]);
+          atomicOr(&p.V[v >> 5], bit);
+        }
+        if (disc) p.lvl[o] = 1;
+        c.mf += dg;
+        c.nnew += disc ? 1u : 0u;
+        wl_append(sh, p.WL[1], &ctrl->wlc[ci], v >> 5, disc && old == 0u, lane);
       }
+      c.unv = 0ull - c.nnew;
+      if (gwarp == 0 && lane == 0) {
+        c.unv += unvAll;
+        c.qbytes += 8ull + 4ull * srcDeg;
+      }
+      wl_flush(sh, p.WL[1], &ctrl->wlc[ci]);
+      block_accumulate(sh, c, ctrl, ci);
+      grid_barrier(&ctrl->bar, epoch);
+      if (leader) tStage1 = globaltimer();
+    } else if (bottomUp) {
       bu_level(p, sh, level, Fp, Fn, Fs, p.WL[level & 1u], ctrl, ci, nu);
       grid_barrier(&ctrl->bar, epoch);
       if (leader) tStage1 = globaltimer();
     } else {
-      if (level == 1) prefill_out();  // the stores drain while the (latency-bound) first expansion runs
       const Marks mk{p.V, Fn, p.hubFilter || mf > 4ull * nu, sh.hub, p.hubFilter ? HUB_BITS : 0u};
       if (p.hubFilter) {
         for (uint32_t i = threadIdx.x; i < HUB_BITS / 32; i += blockDim.x) sh.hub[i] = 0;
@@ -970,7 +998,6 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       }
       td_phase_a<CONTR>(p, sh, p.WL[(level - 1) & 1u], wlCount, Fp, mk, ctrl, ci);
       grid_barrier(&ctrl->bar, epoch);
-      if (level == 1 && leader) p.lvl[p.srcLvl] = 0;  // L[src] = 0 (after the fill: ordered by the barrier)
       if (threadIdx.x == 0) sh.ctl[0] = ld_volatile(&ctrl->qc[ci]);
       __syncthreads();
       const uint32_t nChunks = (uint32_t)sh.ctl[0];
