@@ -59,6 +59,9 @@ struct blest_graph {
   uint32_t* dIso = nullptr;
   uint16_t* dPopThr = nullptr;
   std::vector<uint32_t> isoBits;  // host bitmap of zero-degree vertices (internal ids): such a source reaches nothing
+  std::vector<uint32_t> hubComp;  // host bitmap of the connected component of the highest-degree vertex
+  uint32_t* dOutside = nullptr;   // device bitmap: NOT in that component (zero-degree vertices included)
+  uint32_t nOutsideInSweep = 0;
   uint32_t *dV = nullptr, *dF[3] = {nullptr, nullptr, nullptr}, *dWL[2] = {nullptr, nullptr};
   uint4* dChunks = nullptr;
   uint2* dQ[2] = {nullptr, nullptr};
@@ -291,6 +294,45 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
       uint32_t iso = 0;
       for (uint32_t w = 0; w < g->nSweepWords; ++w) iso += (uint32_t)__builtin_popcount(g->isoBits[w]);
       g->nIsoInSweep = iso;
+      // Connected component of the highest-degree vertex (level-synchronous host BFS, OpenMP over the frontier).  A
+      // traversal from a source inside it can never leave it, so the lazy kernel starts with everything outside marked
+      // visited: no sweep ever examines those vertices, and the traversal ends as soon as the component is exhausted.
+      if (!hostOnly && any) {
+        uint32_t hub = 0, best = 0;
+        for (uint32_t u = 0; u < g->n; ++u) {
+          const uint32_t d = gcsr->rowptr[u + 1] - gcsr->rowptr[u];
+          if (d > best) { best = d; hub = u; }
+        }
+        g->hubComp.assign(g->nwords, 0u);
+        std::vector<uint32_t> frontier{hub}, next;
+        g->hubComp[hub >> 5] |= 1u << (hub & 31u);
+        while (!frontier.empty()) {
+          next.clear();
+#pragma omp parallel
+          {
+            std::vector<uint32_t> mine;
+#pragma omp for schedule(dynamic, 256) nowait
+            for (int64_t i = 0; i < (int64_t)frontier.size(); ++i) {
+              const uint32_t u = frontier[i];
+              for (uint32_t e = gcsr->rowptr[u]; e < gcsr->rowptr[u + 1]; ++e) {
+                const uint32_t v = gcsr->colidx[e], bit = 1u << (v & 31u);
+                if (g->hubComp[v >> 5] & bit) continue;
+                const uint32_t old = __atomic_fetch_or(&g->hubComp[v >> 5], bit, __ATOMIC_RELAXED);
+                if (!(old & bit)) mine.push_back(v);
+              }
+            }
+#pragma omp critical
+            next.insert(next.end(), mine.begin(), mine.end());
+          }
+          frontier.swap(next);
+        }
+        uint32_t outside = 0;
+        for (uint32_t w = 0; w < g->nSweepWords; ++w) {
+          const uint32_t valid = (w == g->nwords - 1 && (g->n & 31u)) ? ((1u << (g->n & 31u)) - 1u) : 0xFFFFFFFFu;
+          outside += (uint32_t)__builtin_popcount(~g->hubComp[w] & valid);
+        }
+        g->nOutsideInSweep = outside;
+      }
     }
     // scale-free-like test in the spirit of PAPER.md:199 (fn. 2: the top 1 % of the vertices hold a large share of the
     // degree); only meaningful after the degree sort, where the top vertices are the first ones
@@ -356,6 +398,15 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
         if ((rc = dev_alloc(g, &g->dDeg, g->n))) return rc;
         if ((rc = dev_alloc(g, &g->dIso, (uint64_t)g->nwords + 16, true))) return rc;
         CK(cudaMemcpy(g->dIso, g->isoBits.data(), (size_t)g->nwords * 4, cudaMemcpyHostToDevice));
+        if (!g->hubComp.empty()) {
+          std::vector<uint32_t> outside(g->nwords);
+          for (uint32_t w = 0; w < g->nwords; ++w) {
+            const uint32_t valid = (w == g->nwords - 1 && (g->n & 31u)) ? ((1u << (g->n & 31u)) - 1u) : 0xFFFFFFFFu;
+            outside[w] = ~g->hubComp[w] & valid;
+          }
+          if ((rc = dev_alloc(g, &g->dOutside, (uint64_t)g->nwords + 16, true))) return rc;
+          CK(cudaMemcpy(g->dOutside, outside.data(), (size_t)g->nwords * 4, cudaMemcpyHostToDevice));
+        }
         if ((rc = dev_alloc(g, &g->dPopThr, (uint64_t)g->nwords + 16))) return rc;
         CK(cudaMemcpy(g->dHead, head.data(), (size_t)g->n * sizeof(uint2), cudaMemcpyHostToDevice));
         CK(cudaMemcpy(g->dDeg, deg.data(), (size_t)g->n * 4, cudaMemcpyHostToDevice));
@@ -464,6 +515,13 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
   p.perm = h->hasPerm ? h->dPerm : nullptr;
   p.iperm = h->hasPerm ? h->dIperm : nullptr;
   p.nSweepWords = h->nSweepWords; p.nIsoInSweep = h->nIsoInSweep; p.isoBits = h->dIso;
+  {  // source inside the hub's component: everything outside starts out visited (zero-degree vertices are outside too)
+    const uint32_t is = h->hasPerm ? h->perm[src] : src;
+    if (h->dOutside && ((h->hubComp[is >> 5] >> (is & 31u)) & 1u)) {
+      p.isoBits = h->dOutside;
+      p.nIsoInSweep = h->nOutsideInSweep;
+    }
+  }
   p.V = h->dV; p.F[0] = h->dF[0]; p.F[1] = h->dF[1]; p.F[2] = h->dF[2];
   p.WL[0] = h->dWL[0]; p.WL[1] = h->dWL[1];
   p.chunks = h->dChunks; p.chunkCap = h->chunkCap;

@@ -935,6 +935,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     const uint32_t wlCount = (uint32_t)sh.ctl[3];
     __syncthreads();
     if (nf == 0) break;  // empty frontier ("terminates at the first level with x = 0")
+    if (unvAll == 0) break;  // nothing left that could be discovered (everything outside the component is pre-marked)
     degVisited += mf;
     const unsigned long long nu = unvAll;  // zero-degree vertices count as visited from the start
     const unsigned long long mu = p.nnz > degVisited ? p.nnz - degVisited : 0ull;
