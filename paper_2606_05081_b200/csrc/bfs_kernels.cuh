@@ -86,7 +86,9 @@ struct MsParams {
   int kappa;
 };
 
-cudaError_t launch_bfs_lazy(const BfsParams& p, int gridBlocks, cudaStream_t st);
+// persistPtr/persistBytes: optional persisting-L2 access-policy window of this launch (levels_out), nullptr/0 = none
+cudaError_t launch_bfs_lazy(const BfsParams& p, int gridBlocks, cudaStream_t st, const void* persistPtr, size_t persistBytes,
+                            float hitRatio);
 cudaError_t launch_bfs_eager(const BfsParams& p, int gridBlocks, cudaStream_t st);
 cudaError_t launch_isolated_source(int32_t* out, uint32_t n, uint32_t src, cudaStream_t st);
 cudaError_t launch_msbfs(const MsParams& p, int gridBlocks, cudaStream_t st);

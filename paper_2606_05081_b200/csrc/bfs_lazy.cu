@@ -1063,20 +1063,44 @@ int coop_blocks(K kernel) {
 }
 
 template <class K>
-cudaError_t coop_launch(K kernel, const BfsParams& p, int gridBlocks, cudaStream_t st) {
+cudaError_t coop_launch(K kernel, const BfsParams& p, int gridBlocks, cudaStream_t st, const void* persistPtr,
+                        size_t persistBytes, float hitRatio) {
   void* args[] = {(void*)&p};
   // the hub bitmap is the last member: without the filter the launch leaves that shared memory to the L1
   const size_t smem = p.hubFilter ? sizeof(LazyShared) : offsetof(LazyShared, hub);
-  return cudaLaunchCooperativeKernel((const void*)kernel, dim3(gridBlocks), dim3(BLOCK_THREADS), args, smem, st);
+  // cooperative launch; the persisting-L2 window (if any) is an attribute of THIS launch, the stream is left alone
+  cudaLaunchAttribute attrs[2];
+  unsigned int na = 0;
+  attrs[na].id = cudaLaunchAttributeCooperative;
+  attrs[na].val.cooperative = 1;
+  ++na;
+  if (persistPtr && persistBytes) {
+    attrs[na].id = cudaLaunchAttributeAccessPolicyWindow;
+    attrs[na].val.accessPolicyWindow.base_ptr = const_cast<void*>(persistPtr);
+    attrs[na].val.accessPolicyWindow.num_bytes = persistBytes;
+    attrs[na].val.accessPolicyWindow.hitRatio = hitRatio;
+    attrs[na].val.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+    attrs[na].val.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+    ++na;
+  }
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(gridBlocks);
+  cfg.blockDim = dim3(BLOCK_THREADS);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cfg.attrs = attrs;
+  cfg.numAttrs = na;
+  return cudaLaunchKernelExC(&cfg, (const void*)kernel, args);
 }
 
 }  // namespace
 
-cudaError_t launch_bfs_lazy(const BfsParams& p, int gridBlocks, cudaStream_t st) {
+cudaError_t launch_bfs_lazy(const BfsParams& p, int gridBlocks, cudaStream_t st, const void* persistPtr, size_t persistBytes,
+                            float hitRatio) {
   switch (p.contraction) {
-    case 2: return coop_launch(bfs_lazy_kernel<2>, p, gridBlocks, st);
-    case 3: return coop_launch(bfs_lazy_kernel<3>, p, gridBlocks, st);
-    default: return coop_launch(bfs_lazy_kernel<1>, p, gridBlocks, st);
+    case 2: return coop_launch(bfs_lazy_kernel<2>, p, gridBlocks, st, persistPtr, persistBytes, hitRatio);
+    case 3: return coop_launch(bfs_lazy_kernel<3>, p, gridBlocks, st, persistPtr, persistBytes, hitRatio);
+    default: return coop_launch(bfs_lazy_kernel<1>, p, gridBlocks, st, persistPtr, persistBytes, hitRatio);
   }
 }
 
