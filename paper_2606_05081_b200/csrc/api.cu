@@ -426,7 +426,9 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
       for (int k = 0; k < 2; ++k)
         if ((rc = dev_alloc(g, &g->dWL[k], (uint64_t)g->nSweepWords + 16384))) return rc;
       // every deferred segment owns more than BIG_EDGES edges / BIG_QUADS quads of its own => exact capacity bounds
-      g->chunkCap = (uint32_t)(g->nnz / CHUNK_EDGES + g->nQuads / CHUNK_QUADS + g->nnz / BIG_EDGES + g->nQuads / BIG_QUADS + 16);
+      // (with one word per warp the thresholds are lower, but then there are at most 36 segments per warp of the grid)
+      g->chunkCap = (uint32_t)(g->nnz / CHUNK_EDGES + g->nQuads / CHUNK_QUADS + g->nnz / BIG_EDGES + g->nQuads / BIG_QUADS + 16 +
+                               36ull * 32ull * 1024ull);
       if ((rc = dev_alloc(g, &g->dChunks, g->chunkCap))) return rc;
       if ((rc = dev_alloc(g, &g->dQ[0], g->qcap))) return rc;
       if ((rc = dev_alloc(g, &g->dQ[1], g->qcap))) return rc;

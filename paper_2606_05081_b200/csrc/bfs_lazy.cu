@@ -317,6 +317,9 @@ __device__ __forceinline__ void td_phase_a(const BfsParams& p, LazyShared& sh, c
   // over the grid (one word per warp below nwarps words)
   const uint32_t W = min(32u, max(1u, (wlCount + nwarps - 1) / nwarps));
   const bool coarse = wlCount >= nwarps;
+  // one word per warp (tiny frontier): segments beyond one batch of a lane set go to the balanced phase, so that no
+  // single warp walks thousands of edges while the grid waits
+  const uint32_t bigEdges = W == 1u ? 128u : BIG_EDGES, bigQuads = W == 1u ? 32u : BIG_QUADS;
   Counters c;
   for (uint32_t i0 = gwarp * W; i0 < wlCount; i0 += nwarps * W) {
     const uint32_t i = i0 + lane;
@@ -362,15 +365,15 @@ __device__ __forceinline__ void td_phase_a(const BfsParams& p, LazyShared& sh, c
         if (!__any_sync(FULL, nq[k] != 0)) continue;
         const uint32_t alpha = (fw >> (8 * k)) & 0xFFu;
         // hub sets -> balanced phase; with an MMA contraction every set is walked by the whole warp (uniform alpha)
-        uint32_t big = __ballot_sync(FULL, nq[k] > (CONTR == 1 ? BIG_QUADS : 0u));
+        uint32_t big = __ballot_sync(FULL, nq[k] > (CONTR == 1 ? bigQuads : 0u));
         while (big) {
           const int src = __ffs(big) - 1;
           big &= big - 1;
           const uint32_t A = __shfl_sync(FULL, a[k], src), NQ = __shfl_sync(FULL, nq[k], src), AL = __shfl_sync(FULL, alpha, src);
-          if (NQ > BIG_QUADS) emit_chunks(p, ctrl, ci, 0u, A, NQ, AL, lane, coarse);
+          if (NQ > bigQuads) emit_chunks(p, ctrl, ci, 0u, A, NQ, AL, lane, coarse);
           else warp_slices<CONTR>(p, Fn, A, NQ, AL, lane);
         }
-        if (CONTR == 1) expand_slices(p, Fn, a[k], nq[k] > BIG_QUADS ? 0u : nq[k], alpha, lane);
+        if (CONTR == 1) expand_slices(p, Fn, a[k], nq[k] > bigQuads ? 0u : nq[k], alpha, lane);
       }
     }
     // ---- CUDA-core edge path: up to four frontier vertices per lane and round
@@ -391,13 +394,13 @@ __device__ __forceinline__ void td_phase_a(const BfsParams& p, LazyShared& sh, c
       for (int q = 0; q < 4; ++q) {
         if (!__any_sync(FULL, deg[q] != 0)) continue;
         c.qbytes += 4ull * deg[q];
-        uint32_t big = __ballot_sync(FULL, deg[q] > BIG_EDGES);
+        uint32_t big = __ballot_sync(FULL, deg[q] > bigEdges);
         while (big) {
           const int src = __ffs(big) - 1;
           big &= big - 1;
           emit_chunks(p, ctrl, ci, 1u, __shfl_sync(FULL, r0[q], src), __shfl_sync(FULL, deg[q], src), 0u, lane, coarse);
         }
-        expand_edges(p, Fn, r0[q], deg[q] > BIG_EDGES ? 0u : deg[q], lane);
+        expand_edges(p, Fn, r0[q], deg[q] > bigEdges ? 0u : deg[q], lane);
       }
     }
   }
