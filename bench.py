@@ -2,6 +2,7 @@
 """bench.py -- the measurement contract of this repo.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config c4_rmat24] [--shrink S]
+                    [--no-parity] [--no-cpu-baseline] [--no-extra]
 
 One "step" = one pass of the whole hot path (blest_bfs: init -> per-level contraction / switch -> lazy finalisation ->
 hand-off, Alg. 2-4) over one batch of synthetic input = single-source BFS from each of the config's seeded
@@ -10,16 +11,28 @@ edge factor 32, degree-sorted before the BVSS build, 64 sources): the config the
 on; it fits one GPU.  blest_build (reorder + BVSS build + upload) is timed separately, as the paper does (Table 7).
 
 Prints ONE JSON line (rank 0).  `value` = GTEPS = (sum over timed BFS calls of the undirected edges of the source's
-component) / device time, inputs resident in HBM.  `e2e` = the same through the C ABI with a pinned HOST levels_out
-buffer (device->host copy of the 4n-byte level array inside the timed region; the only per-call input is the
-4-byte source id).  `roofline` is for the persistent traversal kernel (the only kernel of the step).
+component, taken from the ORACLE's levels) / device time, inputs resident in HBM.  `e2e` = the same through the C ABI
+with a pinned HOST levels_out buffer (device->host copy of the 4n-byte level array inside the timed region; the only
+per-call input is the 4-byte source id).  `roofline` is for the persistent traversal kernel (the only kernel of the
+step).  Outside the timed region the run checks itself: farness / reach of EVERY timed source and the full level
+arrays of four of them against the CPU oracle (`parity_checked`; a mismatch prints the line and exits 1).
+
+The default run (config c4_rmat24, N = 1) also carries, under `config.extra`, the other two components of
+BASELINE.json's metric and row A5's own number: multi-source BFS sources/s on config 5 (kappa = 64, its own roofline
+against a measured L2 peak, its own oracle baseline and parity sample), the forced BVSS slice path (`switching = off`:
+the paper's kernel without Eq. 6) on 8 of the headline sources with its HBM fraction, and the in-repo tensor-pipe /
+barrier / L2 microbenchmarks.  `--config c5_rmat18` makes the multi-source measurement the main line.
+
 `--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores on a bounded sample.
-N > 1: single-source BFS does not shard (replicas only) -- every rank holds the graph and runs
-a disjoint slice of the sources' work; no data-path collective.
+N > 1 (torchrun): single-source BFS does not shard (replicas only): every rank holds the graph
+and traverses from its OWN seeded draw of 64 sources (disjoint work, fixed per rank => weak scaling, no data-path
+collective).  Closeness (config 5) partitions the SOURCES over the ranks as the paper does and sums the
+partial target-side farness arrays with one NCCL all-reduce (fixed total work => strong scaling).
 """
 from __future__ import annotations
 
 import argparse
+import concurrent.futures
 import json
 import os
 import subprocess
@@ -54,6 +67,15 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def committed_profile(key: str):
+    """Per-launch ncu figures of the committed capture of this workload (profiles/traffic.json), or None."""
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(tp)).get(key)
+    except Exception:
+        return None
+
+
 def load_graph(name: str, shrink: int, rank: int, world: int):
     """Rank 0 generates (seeded); with several ranks the CSR is handed over through /dev/shm."""
     if world == 1:
@@ -80,10 +102,18 @@ def load_graph(name: str, shrink: int, rank: int, world: int):
     return n, rp, ci
 
 
-def rank_sources(srcs_all: np.ndarray, rank: int, world: int) -> np.ndarray:
-    """Replicas only: every rank traverses from ALL the config's sources (fixed per-rank work => weak
-    scaling), rotated by rank so that the ranks do not run the identical sequence at the same time."""
-    return np.roll(srcs_all, -rank * max(1, len(srcs_all) // max(world, 1)))
+def rank_sources(name: str, rowptr: np.ndarray, rank: int) -> np.ndarray:
+    """Single-source BFS does not shard (replicas only): rank r traverses from its own seeded draw of the config's
+    number of sources (rank 0: the config's sources), so the ranks do disjoint work of fixed size (weak scaling)."""
+    return gg.config_sources(name, rowptr, replica=rank)
+
+
+def source_range(n: int, rank: int, world: int):
+    """Closeness partitions the sources over the ranks: contiguous, kappa-aligned ranges covering 0..n-1."""
+    per = -(-n // world)
+    per = -(-per // 256) * 256  # whole batches for every kappa
+    first = min(rank * per, n)
+    return first, min(per, n - first)
 
 
 class ClockSampler:
@@ -158,6 +188,94 @@ def w_alg_bytes(trace: np.ndarray, n: int, reach: int, reordered: bool, sweep_wo
     return int(w)
 
 
+def ms_alg_bytes(stats: dict, kappa: int, n_slice_sets: int, n: int, accumulate: bool) -> int:
+    """Algorithmic bytes of one multi-source launch (all batches), from the kernel's own totals (blest_get_ms_stats);
+    everything is L2-resident on config 5.  KB = kappa / 8 bytes per kappa-bit word.
+    Stage 1, per work-queue entry (VSS): 8 B entry + the 8 gathered frontier words (8 KB); per quad 20 B (row ids + masks);
+      per slice whose selected frontier words are non-zero: one V_next probe (KB); per fresh row: one atomic OR (KB) +
+      the dirtySets byte;
+    Stage 2, per level: the dirtySets sweep (1 B per slice set); per dirty slice set: 8 rows x (V_next + V_curr read,
+      F_curr + V_curr written: 4 KB) + 8 B setPtr + a queue entry per 32 quads (counted with Stage 1) + 12 B per row of
+      far / reach accumulation;
+    per batch: V_curr and V_next cleared (2 x n KB)."""
+    kb = kappa // 8
+    w = stats["entries"] * (8 + 8 * kb) + stats["quads"] * 20 + stats["probes"] * kb + stats["fresh"] * (kb + 1)
+    w += (stats["levels"] + stats["batches"]) * n_slice_sets
+    w += stats["dirty_sets"] * (8 * 4 * kb + 8 + (8 * 12 if accumulate else 0))
+    w += stats["batches"] * 2 * n * kb
+    return int(w)
+
+
+# ----------------------------------------------------------------------------------------------------------------------
+# CPU oracle legs (rank 0 only; outside every timed GPU region)
+# ----------------------------------------------------------------------------------------------------------------------
+def oracle_bfs_checks(n, rp, ci, srcs, deg, gpu_far, gpu_reach, gpu_levels, want_baseline: bool):
+    """cpu_baseline + parity of the single-source workload.  The oracle (as it stands) runs one plain queue BFS per
+    OpenMP thread: the first min(cores, #sources) sources are TIMED (the reported CPU baseline), the rest run untimed.
+    Every source's (farness, reach) is compared with the sums of the GPU's level array; the sources in `gpu_levels`
+    are compared element by element.  Returns (cpu_baseline dict | None, parity dict, per-source oracle edge counts)."""
+    import oracle
+
+    cores = os.cpu_count() or 1
+    k = int(min(cores, len(srcs)))
+    t0 = time.perf_counter()
+    far0, reach0, _, used = oracle.closeness(n, rp, ci, srcs[:k], nthreads=k)
+    dt = time.perf_counter() - t0
+    far, reach = [int(x) for x in far0], [int(x) for x in reach0]
+    if len(srcs) > k:
+        f1, r1, _, _ = oracle.closeness(n, rp, ci, srcs[k:])
+        far += [int(x) for x in f1]
+        reach += [int(x) for x in r1]
+    # element-wise: the oracle's level arrays of a few sources (threads: the C call releases the GIL)
+    idx = sorted(gpu_levels)
+    with concurrent.futures.ThreadPoolExecutor(max(1, len(idx))) as ex:
+        ref = dict(zip(idx, ex.map(lambda i: oracle.bfs(n, rp, ci, int(srcs[i])), idx)))
+    bad_far = [int(srcs[i]) for i in range(len(srcs)) if (far[i], reach[i]) != (int(gpu_far[i]), int(gpu_reach[i]))]
+    bad_lv = [int(srcs[i]) for i in idx if not np.array_equal(ref[i], gpu_levels[i])]
+    # TEPS numerators from the ORACLE's levels: a source inside the component of a reference array shares its edge count
+    edges = np.zeros(len(srcs), dtype=np.int64)
+    comps = [(lv, component_edges(deg, lv)) for lv in ref.values()]
+    for i, s in enumerate(srcs):
+        e = next((ce for lv, ce in comps if lv[int(s)] >= 0), None)
+        if e is None:
+            lv = oracle.bfs(n, rp, ci, int(s))
+            e = component_edges(deg, lv)
+            comps.append((lv, e))
+        edges[i] = e
+    parity = {"sources": int(len(srcs)), "elementwise": int(len(idx)), "ok": not bad_far and not bad_lv,
+              "what": "levels of every timed source: farness + reach vs oracle; `elementwise` sources: full int32 level array"}
+    if bad_far or bad_lv:
+        parity["mismatch_sources"] = (bad_far + bad_lv)[:8]
+    base = None
+    if want_baseline:
+        base = {"value": float(edges[:k].sum() / dt / 1e9), "unit": "GTEPS", "cores": int(used), "kind": "oracle", "seconds": dt,
+                "sample": f"first {k} of the config's {len(srcs)} sources, one plain queue BFS per OpenMP thread"}
+    return base, parity, edges
+
+
+def oracle_closeness_checks(n, rp, ci, cc_gpu: np.ndarray, budget_s: float = 12.0):
+    """cpu_baseline + parity of the closeness workload: the oracle (all host threads, one BFS per source) on a seeded
+    sample sized to ~budget_s; its fp64 closeness must equal the GPU's bit for bit on that sample."""
+    import oracle
+
+    rng = np.random.Generator(np.random.PCG64(5))
+    probe = np.sort(rng.choice(n, size=min(n, 256), replace=False)).astype(np.uint32)
+    t0 = time.perf_counter()
+    _, _, cc_p, used = oracle.closeness(n, rp, ci, probe)
+    t_probe = time.perf_counter() - t0
+    k = int(min(n, max(256, budget_s / max(t_probe, 1e-6) * probe.size)))
+    sample = np.sort(rng.choice(n, size=k, replace=False)).astype(np.uint32)
+    t0 = time.perf_counter()
+    _, _, cc_w, used = oracle.closeness(n, rp, ci, sample)
+    dt = time.perf_counter() - t0
+    ok = bool(np.array_equal(cc_gpu[sample], cc_w) and np.array_equal(cc_gpu[probe], cc_p))
+    base = {"value": float(k / dt), "unit": "sources/s", "cores": int(used), "kind": "oracle", "seconds": dt,
+            "sample": f"{k} seeded sources of the config's {n}, one plain queue BFS + farness per source, sources over all OpenMP threads"}
+    parity = {"sources": int(k + probe.size), "elementwise": int(k + probe.size), "ok": ok,
+              "what": "fp64 closeness of the sampled sources, bit-equal to the oracle's"}
+    return base, parity
+
+
 def run_reference(args, rank: int, world: int):
     """--impl reference: the CPU oracle as it stands, on the host cores, bounded sample per step."""
     if rank != 0:
@@ -165,39 +283,207 @@ def run_reference(args, rank: int, world: int):
     import oracle
 
     n, rp, ci = gg.make_config(args.config, args.shrink)
-    srcs_all = gg.config_sources(args.config, rp)
     cores = os.cpu_count() or 1
-    deg = gg.degrees(rp)
-    # calibrate the sample: one source on one thread, then size a step to ~budget seconds
-    t0 = time.perf_counter()
-    lv = oracle.bfs(n, rp, ci, int(srcs_all[0]))
-    t_one = time.perf_counter() - t0
-    budget = 150.0 / max(1, args.steps + args.warmup)
-    k = int(max(1, min(len(srcs_all), cores, budget / max(t_one, 1e-6) * cores / 2.5)))
-    sample = srcs_all[:k]
-    edges = 0
-    for s in sample:
-        edges += component_edges(deg, lv if s == srcs_all[0] else oracle.bfs(n, rp, ci, int(s)))
-    used = 1
-    for _ in range(args.warmup):
-        _, _, _, used = oracle.closeness(n, rp, ci, sample, nthreads=k)
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        _, _, _, used = oracle.closeness(n, rp, ci, sample, nthreads=k)
-    dt = time.perf_counter() - t0
-    gteps = edges * args.steps / dt / 1e9
+    if args.config == "c5_rmat18":
+        rng = np.random.Generator(np.random.PCG64(5))
+        probe = rng.choice(n, size=min(n, 64), replace=False).astype(np.uint32)
+        t0 = time.perf_counter()
+        oracle.closeness(n, rp, ci, probe)
+        t_one = (time.perf_counter() - t0) / probe.size
+        budget = 150.0 / max(1, args.steps + args.warmup)
+        k = int(max(cores, min(n, budget / max(t_one, 1e-9))))
+        sample = np.sort(rng.choice(n, size=k, replace=False)).astype(np.uint32)
+        used = 1
+        for _ in range(args.warmup):
+            _, _, _, used = oracle.closeness(n, rp, ci, sample)
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            _, _, _, used = oracle.closeness(n, rp, ci, sample)
+        dt = time.perf_counter() - t0
+        val, unit, metric = k * args.steps / dt, "sources/s", "msbfs_sources_per_s"
+        desc = f"{k} seeded sources per step, one plain queue BFS + farness per source over all OpenMP threads, {args.steps} steps"
+        cfg = {"workload": args.config, "shrink": args.shrink, "n": int(n), "nnz": int(ci.size), "sources_per_step": int(k)}
+    else:
+        srcs_all = gg.config_sources(args.config, rp)
+        deg = gg.degrees(rp)
+        # calibrate the sample: one source on one thread, then size a step to ~budget seconds
+        t0 = time.perf_counter()
+        lv = oracle.bfs(n, rp, ci, int(srcs_all[0]))
+        t_one = time.perf_counter() - t0
+        budget = 150.0 / max(1, args.steps + args.warmup)
+        k = int(max(1, min(len(srcs_all), cores, budget / max(t_one, 1e-6) * cores / 2.5)))
+        sample = srcs_all[:k]
+        edges = 0
+        for s in sample:
+            edges += component_edges(deg, lv if (s == srcs_all[0] or lv[int(s)] >= 0) else oracle.bfs(n, rp, ci, int(s)))
+        used = 1
+        for _ in range(args.warmup):
+            _, _, _, used = oracle.closeness(n, rp, ci, sample, nthreads=k)
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            _, _, _, used = oracle.closeness(n, rp, ci, sample, nthreads=k)
+        dt = time.perf_counter() - t0
+        val, unit, metric = edges * args.steps / dt / 1e9, "GTEPS", "bfs_gteps"
+        desc = (f"{k} of the config's {len(srcs_all)} sources per step, one plain queue BFS per thread "
+                f"(oracle_closeness: BFS + farness), {args.steps} steps")
+        cfg = {"workload": args.config, "shrink": args.shrink, "n": int(n), "nnz": int(ci.size), "sources_per_step": int(k)}
     line = {
-        "impl": "reference", "metric": "bfs_gteps", "value": gteps, "unit": "GTEPS", "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-        "config": {"workload": args.config, "shrink": args.shrink, "n": int(n), "nnz": int(ci.size), "sources_per_step": int(k)},
-        "cpu_baseline": {"value": gteps, "unit": "GTEPS", "cores": int(used), "kind": "oracle",
-                         "sample": f"{k} of the config's {len(srcs_all)} sources per step, one plain queue BFS per thread "
-                                   f"(oracle_closeness: BFS + farness), {args.steps} steps"},
-        "e2e": {"value": gteps, "unit": "GTEPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "impl": "reference", "metric": metric, "value": val, "unit": unit, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "strong" if args.config == "c5_rmat18" else "weak",
+        "vs_baseline": None, "dtype": "int32", "data": "synthetic", "config": cfg,
+        "cpu_baseline": {"value": val, "unit": unit, "cores": int(used), "kind": "oracle", "sample": desc},
+        "e2e": {"value": val, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------------------------------------
+# GPU workloads
+# ----------------------------------------------------------------------------------------------------------------------
+def forced_slice_extra(g, torch, srcs, edges, n, reordered, sweep_words, peak, stream, out):
+    """Row A5's own number in the driver-run record: the BVSS slice path forced through every level (`switching = off`,
+    the paper's Alg. 3 without Eq. 6) on a few of the headline sources: GTEPS and the HBM fraction of its algorithmic
+    bytes.  Levels are compared with the default path's (policy independence) on the fly."""
+    k = min(8, len(srcs))
+    ref = []
+    for s in srcs[:k]:
+        g.bfs(int(s), out, stream=stream)
+        stream.synchronize()
+        ref.append(out.clone())
+    g.configure(switching="off")
+    walg, same = 0, True
+    for i, s in enumerate(srcs[:k]):
+        g.bfs(int(s), out, stream=stream)
+        stream.synchronize()
+        same = same and bool(torch.equal(out, ref[i]))
+        lv_reach = int((out >= 0).sum().item())
+        walg += w_alg_bytes(g.trace(), n, lv_reach, reordered, sweep_words)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = 2
+    e0.record(stream)
+    for _ in range(reps):
+        for s in srcs[:k]:
+            g.bfs(int(s), out, stream=stream)
+    e1.record(stream)
+    stream.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    g.configure(switching="auto")
+    achieved = walg / (ms * 1e-3) / 1e9
+    prof = committed_profile("c4_rmat24/0/switching_off") or {}
+    return {"what": "BVSS slice path on every level (switching=off: PAPER.md Alg. 3 without Eq. 6), ALU contraction",
+            "sources": int(k), "gteps": float(edges[:k].sum() / (ms * 1e-3) / 1e9), "ms_per_bfs": ms / k,
+            "algorithmic_gb_per_bfs": walg / k / 1e9, "achieved_gbs": achieved, "hbm_frac": achieved / peak,
+            "levels_equal_default_path": same, "dram_bytes_per_launch_ncu": prof.get("dram_bytes_per_launch_mean"),
+            "tensor_pipe_active_pct_ncu": prof.get("tensor_pipe_active_pct")}
+
+
+def microbench_extra(blest):
+    """In-repo peaks (north_star: tensor-pipe utilisation is quoted against a peak measured by an in-repo microbenchmark)."""
+    out = {}
+    try:
+        out["mma_sync_b1_tera_bitmacs"] = blest.mma_microbench("mma_b1", 2048)[0]
+        out["mma_sync_u8_tera_bytemacs"] = blest.mma_microbench("mma_u8", 2048)[0]
+        if hasattr(blest, "tcgen05_microbench"):
+            out["tcgen05_i8_tera_bytemacs"] = blest.tcgen05_microbench(2048)[0]
+        out["grid_barrier_ns"] = blest.barrier_microbench(2000)
+        out["l2_copy_gbs"] = blest.l2_microbench(48 << 20, 50)
+    except Exception as e:  # a microbenchmark must not take the headline down
+        out["error"] = repr(e)
+    return out
+
+
+def closeness_measure(args, torch, blest, rank, world, dist, steps, warmup, want_cpu):
+    """Exact closeness of ALL vertices of config 5 (§6.2), kappa bit-packed sources per batch; one step = the
+    whole source set once.  N = 1: one blest_closeness call.  N > 1: rank r runs blest_farness_partial over its source
+    range, one all-reduce sums the partial target-side arrays, blest_closeness_from_sums divides."""
+    n, rp, ci = load_graph("c5_rmat18", args.shrink, rank, world) if args.config == "c5_rmat18" else gg.make_config("c5_rmat18", args.shrink)
+    g = blest.Graph(n, rp, ci, reorder="none", kappa=args.kappa)
+    info = g.info()
+    stream = torch.cuda.current_stream() if world > 1 else torch.cuda.Stream()
+    cc = torch.zeros(n, dtype=torch.float64, device="cuda")
+    host_cc = torch.zeros(n, dtype=torch.float64).pin_memory()
+    far = torch.zeros(n, dtype=torch.int64, device="cuda")
+    reach = torch.zeros(n, dtype=torch.int32, device="cuda")
+    first, count = source_range(n, rank, world)
+
+    def step(dst):
+        if world == 1:
+            g.closeness(dst, stream=stream)
+            return
+        if count:
+            g.farness_partial(first, count, far, reach, stream=stream)
+        else:
+            far.zero_()
+            reach.zero_()
+        dist.all_reduce(far)     # the path's one exchange step (PAPER.md:678): partial sums -> totals, NCCL over NVLink
+        dist.all_reduce(reach)
+        blest.closeness_from_sums(far, reach, cc, stream=stream)
+        if dst is not cc:
+            dst.copy_(cc, non_blocking=True)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    with torch.cuda.stream(stream):
+        for _ in range(max(warmup, 1)):
+            step(cc)
+        barrier()
+        stats = g.ms_stats()
+        sampler = ClockSampler(int(os.environ.get("LOCAL_RANK", "0"))) if rank == 0 else None
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            step(cc)
+        e1.record(stream)
+        barrier()
+        dev_ms = e0.elapsed_time(e1)
+        e0.record(stream)
+        for _ in range(steps):
+            step(host_cc)
+            stream.synchronize()  # the step's result is read on the host
+        e1.record(stream)
+        barrier()
+        e2e_ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if sampler else None
+    if dist is not None:
+        t = torch.tensor([dev_ms, e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dev_ms, e2e_ms = float(t[0]), float(t[1])
+    res = None
+    if rank == 0:
+        l2_peak = blest.l2_microbench(48 << 20, 50)
+        walg = ms_alg_bytes(stats, args.kappa, info.n_slice_sets, n, True)  # this rank's launch
+        achieved = walg / (dev_ms / steps * 1e-3) / 1e9 if world == 1 else None
+        res = {
+            "value": n * steps / (dev_ms * 1e-3), "ms_per_step": dev_ms / steps, "clocks": clocks,
+            "e2e": {"value": n * steps / (e2e_ms * 1e-3), "unit": "sources/s", "h2d_bytes_per_step": 0,
+                    "d2h_bytes_per_step": int(8 * n), "ms_per_step": e2e_ms / steps},
+            "config": {"workload": "c5_rmat18", "shrink": args.shrink, "n": int(n), "nnz": int(ci.size), "kappa": args.kappa,
+                       "batches": (n + args.kappa - 1) // args.kappa,
+                       "l2": "L2-resident graph (the workload re-traverses a 40 MB graph; no flush)",
+                       "bvss_bytes": int(info.bvss_bytes),
+                       "parallelism": "sources partitioned over ranks + all-reduce of the target-side sums" if world > 1 else "1 GPU",
+                       "levels_per_batch": stats["levels"] / max(stats["batches"], 1), "vss_entries_per_step": stats["entries"]},
+            "roofline": {"bound": "l2", "achieved": achieved, "peak": l2_peak, "unit": "GB/s",
+                         "frac": (achieved / l2_peak) if achieved else None, "traffic": None,
+                         "peak_source": "measured: blest_l2_microbench (48 MB footprint copy, persistent launch configuration)",
+                         "kernel": "msbfs_kernel (persistent cooperative; one launch = all batches)",
+                         "algorithmic_bytes_per_launch_mean": float(walg), "ms_per_launch_mean": dev_ms / steps},
+            "gpu_launches": int(steps * (2 if world == 1 else 3)),
+        }
+        prof = committed_profile(f"c5_rmat18/{args.shrink}/kappa{args.kappa}")
+        if prof:
+            res["roofline"]["traffic"] = prof.get("l2_bytes_per_launch_mean")
+            res["roofline"]["traffic_source"] = prof.get("source")
+        if want_cpu:
+            base, parity = oracle_closeness_checks(n, rp, ci, cc.cpu().numpy())
+            res["cpu_baseline"], res["parity_checked"] = base, parity
+    g.close()
+    return res
 
 
 def main():
@@ -208,13 +494,17 @@ def main():
     ap.add_argument("--impl", default="blest", choices=["blest", "reference"])
     ap.add_argument("--config", default="c4_rmat24", choices=sorted(gg.CONFIGS))
     ap.add_argument("--shrink", type=int, default=0, help="halve the linear size this many times (debug only)")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle legs (cpu_baseline AND parity)")
+    ap.add_argument("--no-parity", action="store_true", help="alias of --no-cpu-baseline")
+    ap.add_argument("--no-extra", action="store_true", help="skip config.extra (closeness, forced slice path, microbenchmarks)")
     ap.add_argument("--kernel", default="auto")
     ap.add_argument("--switching", default="auto")
     ap.add_argument("--contraction", default="auto")
+    ap.add_argument("--reorder", default=None)
     ap.add_argument("--kappa", type=int, default=64)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
+    want_cpu = not (args.no_cpu_baseline or args.no_parity)
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -231,9 +521,6 @@ def main():
     import paper_2606_05081_b200 as blest
 
     torch.cuda.set_device(local_rank)
-    if args.config == "c5_rmat18":  # multi-source BFS / closeness: a different metric (sources per second)
-        run_closeness(args, rank, world, torch, blest)
-        return
     dist = None
     if world > 1:
         import torch.distributed as dist
@@ -242,15 +529,31 @@ def main():
         os.environ.setdefault("OMP_NUM_THREADS", str(max(1, (os.cpu_count() or 1) // world)))
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
+    if args.config == "c5_rmat18":  # multi-source BFS / closeness: the metric's third component as the main line
+        res = closeness_measure(args, torch, blest, rank, world, dist, args.steps, args.warmup, want_cpu)
+        if rank == 0:
+            line = {"metric": "msbfs_sources_per_s", "value": res["value"], "unit": "sources/s", "n_gpus": world,
+                    "steps": args.steps, "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True,
+                    "scaling": "strong" if world > 1 else "weak", "vs_baseline": None, "dtype": "u%d" % args.kappa,
+                    "data": "synthetic", "config": res["config"], "e2e": res["e2e"], "gpu_launches": res["gpu_launches"],
+                    "clocks": res["clocks"], "roofline": res["roofline"]}
+            for k in ("cpu_baseline", "parity_checked"):
+                if k in res:
+                    line[k] = res[k]
+            print(json.dumps(line), flush=True)
+            if "parity_checked" in res and not res["parity_checked"]["ok"]:
+                sys.exit(1)
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+
     t0 = time.perf_counter()
     n, rp, ci = load_graph(args.config, args.shrink, rank, world)
     gen_s = time.perf_counter() - t0
     deg = gg.degrees(rp)
-    srcs_all = gg.config_sources(args.config, rp)
-    # replicas only: every rank traverses the full graph; rank r takes the sources rotated by r so that the ranks do
-    # not run the identical sequence.  Per-rank work is fixed as N grows => weak scaling.
-    srcs = rank_sources(srcs_all, rank, world)
-    reorder = REORDER_FOR[args.config]
+    srcs = rank_sources(args.config, rp, rank)
+    reorder = args.reorder or REORDER_FOR[args.config]
     log(f"[rank {rank}] {args.config} shrink {args.shrink}: n={n} nnz={ci.size} gen {gen_s:.1f}s; building (reorder={reorder})")
     t0 = time.perf_counter()
     g = blest.Graph(n, rp, ci, reorder=reorder, kernel=args.kernel, switching=args.switching, contraction=args.contraction)
@@ -258,22 +561,33 @@ def main():
     info = g.info()
     stream = torch.cuda.Stream()
     out = torch.empty(n, dtype=torch.int32, device="cuda")
+    out2 = torch.empty(n, dtype=torch.int32, device="cuda")
     host_out = torch.empty(n, dtype=torch.int32).pin_memory()
+    host_out2 = torch.empty(n, dtype=torch.int32).pin_memory()
 
-    # per-source numerators + algorithmic bytes from one untimed pass (also warm-up #0)
+    # one untimed pass (also warm-up #0): per-source sums of the GPU's level array, algorithmic bytes from the trace
     sweep_words = int(info.n_sweep_words)
-    edges = np.zeros(len(srcs), dtype=np.int64)
+    gpu_edges = np.zeros(len(srcs), dtype=np.int64)
+    gpu_far = np.zeros(len(srcs), dtype=np.int64)
+    gpu_reach = np.zeros(len(srcs), dtype=np.int64)
     walg = np.zeros(len(srcs), dtype=np.int64)
     nlevels = np.zeros(len(srcs), dtype=np.int64)
+    keep = {}  # GPU level arrays of the sources compared element by element
+    elementwise = set(np.linspace(0, len(srcs) - 1, num=min(4, len(srcs)), dtype=int).tolist())
     with torch.cuda.stream(stream):
         for i, s in enumerate(srcs):
             g.bfs(int(s), out, stream=stream)
             stream.synchronize()
             lv = out.cpu().numpy()
-            edges[i] = component_edges(deg, lv)
+            reached = lv >= 0
+            gpu_edges[i] = int(deg[reached].sum() // 2)
+            gpu_reach[i] = int(reached.sum())
+            gpu_far[i] = int(lv[reached].astype(np.int64).sum())
+            if i in elementwise:
+                keep[i] = lv.copy()
             tr = g.trace()
             nlevels[i] = len(tr)
-            walg[i] = w_alg_bytes(tr, n, int((lv >= 0).sum()), reorder != "none", sweep_words)
+            walg[i] = w_alg_bytes(tr, n, int(gpu_reach[i]), reorder != "none", sweep_words)
 
     def one_step(dst, evs=None):
         for i, s in enumerate(srcs):
@@ -316,22 +630,55 @@ def main():
     e1.record(stream)
     barrier()
     e2e_ms = e0.elapsed_time(e1)
+    # e2e, overlapped by the caller: device output buffers alternate, the device->host copy of BFS i runs on a second
+    # stream while BFS i+1 traverses (still 4n bytes to the host per BFS; the PCIe copy is the bound)
+    copy_stream = torch.cuda.Stream()
+    dbuf, hbuf = (out, out2), (host_out, host_out2)
+    done = [torch.cuda.Event(), torch.cuda.Event()]
+    freed = [torch.cuda.Event(), torch.cuda.Event()]
+    e0.record(stream)
+    j = 0
+    for k in range(args.steps):
+        for s in srcs:
+            b = j & 1
+            if j >= 2:
+                stream.wait_event(freed[b])
+            g.bfs(int(s), dbuf[b], stream=stream)
+            done[b].record(stream)
+            copy_stream.wait_event(done[b])
+            with torch.cuda.stream(copy_stream):
+                hbuf[b].copy_(dbuf[b], non_blocking=True)
+                freed[b].record(copy_stream)
+            j += 1
+    stream.wait_stream(copy_stream)
+    e1.record(stream)
+    barrier()
+    e2e_ov_ms = e0.elapsed_time(e1)
     clocks = sampler.stop() if sampler else None
 
-    t_max, e2e_max = dev_ms, e2e_ms
-    if dist is not None:
-        t = torch.tensor([dev_ms, e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_max, e2e_max = float(t[0]), float(t[1])
-    total_edges = int(edges.sum()) * args.steps * world
-    gteps = total_edges / (t_max * 1e-3) / 1e9
-    e2e_gteps = total_edges / (e2e_max * 1e-3) / 1e9
+    # oracle legs (rank 0): cpu_baseline + parity + TEPS numerators from the oracle's levels
+    base, parity, edges = None, None, gpu_edges
+    if rank == 0 and want_cpu:
+        base, parity, edges = oracle_bfs_checks(n, rp, ci, srcs, deg, gpu_far, gpu_reach, keep, True)
 
+    t_max, e2e_max, e2e_ov_max, edge_sum = dev_ms, e2e_ms, e2e_ov_ms, float(edges.sum())
+    if dist is not None:
+        t = torch.tensor([dev_ms, e2e_ms, e2e_ov_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        t_max, e2e_max, e2e_ov_max = float(t[0]), float(t[1]), float(t[2])
+        es = torch.tensor([edge_sum], device="cuda", dtype=torch.float64)
+        dist.all_reduce(es)  # units all ranks processed (every rank has its own sources)
+        edge_sum = float(es[0])
+    total_edges = edge_sum * args.steps
+    gteps = total_edges / (t_max * 1e-3) / 1e9
+
+    ok = True
     if rank == 0:
         peak, peak_src = measured_peaks()
         med = np.median(per, axis=0)  # per-source median over steps, ms
         giant = edges >= 0.5 * edges.max()
         achieved = float(walg.sum() * args.steps / (per.sum() * 1e-3) / 1e9)  # GB/s, all launches of the timed region
+        prof = committed_profile(f"{args.config}/{args.shrink}") or {}
         line = {
             "metric": "bfs_gteps", "value": gteps, "unit": "GTEPS", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": t_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -339,103 +686,61 @@ def main():
             "config": {
                 "workload": args.config, "shrink": args.shrink, "n": int(n), "nnz": int(ci.size), "reorder": reorder,
                 "sources_per_step": int(len(srcs)), "l2": "inputs larger than L2 (BVSS+CSR >> 126 MB)" if info.bvss_bytes > (1 << 28) else "L2-resident graph (no flush: the paper's workload re-traverses a resident graph)",
-                "kernel": {1: "eager (Alg. 2)", 2: "lazy (Alg. 3) + switching"}[info.kernel_chosen], "parallelism": "replicas only" if world > 1 else "1 GPU",
+                "kernel": {1: "eager (Alg. 2)", 2: "lazy (Alg. 3) + switching"}[info.kernel_chosen],
+                "parallelism": "replicas only (own sources per rank)" if world > 1 else "1 GPU",
+                "teps_numerator": "oracle levels" if parity else "GPU levels (oracle legs skipped)",
                 "bvss_bytes": int(info.bvss_bytes), "csr_bytes": int(info.csr_bytes), "mask_density": info.mask_density, "u_div": info.u_div,
                 "gen_seconds": gen_s, "reorder_seconds": info.reorder_seconds, "bvss_build_seconds": info.build_seconds,
-                "upload_seconds": info.upload_seconds, "build_wall_seconds": build_wall,
+                "component_seconds": info.component_seconds, "upload_seconds": info.upload_seconds, "build_wall_seconds": build_wall,
                 "gteps_harmonic_mean_giant": float(giant.sum() / np.sum((med[giant] * 1e-3) / (edges[giant] / 1e9))) if giant.any() else None,
                 "ms_per_bfs_median": float(np.median(med)), "ms_per_bfs_min": float(med.min()), "ms_per_bfs_max": float(med.max()),
                 "levels_median": float(np.median(nlevels)), "us_per_level": float(np.median(med * 1e3 / np.maximum(nlevels, 1))),
             },
-            "e2e": {"value": e2e_gteps, "unit": "GTEPS", "h2d_bytes_per_step": int(4 * len(srcs)),
-                    "d2h_bytes_per_step": int(4 * n * len(srcs)), "ms_per_step": e2e_max / args.steps},
+            "e2e": {"value": total_edges / (e2e_max * 1e-3) / 1e9, "unit": "GTEPS", "h2d_bytes_per_step": int(4 * len(srcs)),
+                    "d2h_bytes_per_step": int(4 * n * len(srcs)), "ms_per_step": e2e_max / args.steps,
+                    "overlapped": {"value": total_edges / (e2e_ov_max * 1e-3) / 1e9, "ms_per_step": e2e_ov_max / args.steps,
+                                   "what": "device levels_out double-buffered by the caller, device->host copy of BFS i on a second stream under BFS i+1"}},
             "gpu_launches": int(args.steps * len(srcs)),
             "clocks": clocks,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "peak_source": peak_src, "kernel": KERNEL_NAME,
+                         "traffic": prof.get("dram_bytes_per_launch_mean"), "traffic_source": prof.get("source"),
+                         "traffic_commit": prof.get("commit"), "peak_source": peak_src, "kernel": KERNEL_NAME,
                          "algorithmic_bytes_per_launch_mean": float(walg.mean()), "ms_per_launch_mean": float(per.mean())},
+            "tensor_pipe": {"active_pct": prof.get("tensor_pipe_active_pct", 0.0),
+                            "note": "the default contraction is the ALU form (no MMA instruction in the timed kernel); the MMA "
+                                    "forms are measured on the forced slice path (profiles/, config.extra)"},
         }
-        tp = os.path.join(ROOT, "profiles", "traffic.json")  # dram bytes per launch from the committed ncu capture
-        if os.path.exists(tp):
+        if parity is not None:
+            line["parity_checked"] = parity
+            ok = parity["ok"]
+        if base is not None:
+            line["cpu_baseline"] = base
+        if world == 1 and not args.no_extra and args.shrink == 0 and args.config == "c4_rmat24":
+            extra = {}
             try:
-                t = json.load(open(tp)).get(f"{args.config}/{args.shrink}")
-                if t:  # bytes per launch, like `achieved`'s numerator
-                    line["roofline"]["traffic"] = float(t["dram_bytes_per_launch_mean"])
-                    line["roofline"]["traffic_source"] = t["source"]
-            except Exception:
-                pass
-        if not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(n, rp, ci, srcs_all, deg)
+                extra["forced_slice_path"] = forced_slice_extra(g, torch, srcs, edges, n, reorder != "none", sweep_words, peak, stream, out)
+            except Exception as e:
+                extra["forced_slice_path"] = {"error": repr(e)}
+            g.close()
+            try:
+                cres = closeness_measure(args, torch, blest, 0, 1, None, 1, 1, want_cpu)
+                extra["msbfs_closeness_c5"] = {"metric": "msbfs_sources_per_s", "value": cres["value"], "unit": "sources/s",
+                                               "ms_per_step": cres["ms_per_step"], "e2e": cres["e2e"], "config": cres["config"],
+                                               "roofline": cres["roofline"], "cpu_baseline": cres.get("cpu_baseline"),
+                                               "parity_checked": cres.get("parity_checked")}
+                if cres.get("parity_checked") and not cres["parity_checked"]["ok"]:
+                    ok = False
+            except Exception as e:
+                extra["msbfs_closeness_c5"] = {"error": repr(e)}
+            extra["microbench"] = microbench_extra(blest)
+            line["config"]["extra"] = extra
         print(json.dumps(line), flush=True)
     g.close()
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
-
-
-def run_closeness(args, rank, world, torch, blest):
-    """--config c5_rmat18: exact closeness of ALL vertices (§6.2), kappa bit-packed sources per batch; one step =
-    one blest_closeness call over all n sources.  Reported as MS-BFS sources per second (BASELINE.json metric).  The
-    graph (40 MB) is L2-resident by nature of the workload.  Replicas only for N > 1."""
-    n, rp, ci = gg.make_config(args.config, args.shrink)
-    g = blest.Graph(n, rp, ci, reorder="none", kappa=args.kappa)
-    info = g.info()
-    stream = torch.cuda.Stream()
-    cc = torch.zeros(n, dtype=torch.float64, device="cuda")
-    host_cc = torch.zeros(n, dtype=torch.float64).pin_memory()
-    for _ in range(max(args.warmup, 1)):
-        g.closeness(cc, stream=stream)
-    torch.cuda.synchronize()
-    sampler = ClockSampler(int(os.environ.get("LOCAL_RANK", "0"))) if rank == 0 else None
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(args.steps):
-        g.closeness(cc, stream=stream)
-    e1.record(stream)
-    torch.cuda.synchronize()
-    dev_ms = e0.elapsed_time(e1)
-    e0.record(stream)
-    for _ in range(args.steps):
-        g.closeness(host_cc, stream=stream)
-    e1.record(stream)
-    torch.cuda.synchronize()
-    e2e_ms = e0.elapsed_time(e1)
-    clocks = sampler.stop() if sampler else None
-    if rank == 0:
-        line = {
-            "metric": "msbfs_sources_per_s", "value": n * args.steps * world / (dev_ms * 1e-3), "unit": "sources/s", "n_gpus": world,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dev_ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "u%d" % args.kappa, "data": "synthetic",
-            "config": {"workload": args.config, "shrink": args.shrink, "n": int(n), "nnz": int(ci.size), "kappa": args.kappa,
-                       "batches": (n + args.kappa - 1) // args.kappa, "l2": "L2-resident graph (the workload re-traverses a 40 MB graph)",
-                       "bvss_bytes": int(info.bvss_bytes), "parallelism": "replicas only" if world > 1 else "1 GPU"},
-            "e2e": {"value": n * args.steps * world / (e2e_ms * 1e-3), "unit": "sources/s", "h2d_bytes_per_step": 0,
-                    "d2h_bytes_per_step": int(8 * n), "ms_per_step": e2e_ms / args.steps},
-            "gpu_launches": int(2 * args.steps), "clocks": clocks,
-        }
-        print(json.dumps(line), flush=True)
-    g.close()
-
-
-def cpu_baseline(n, rp, ci, srcs_all, deg):
-    """The oracle as it stands on the host cores, bounded sample (~10-30 s): min(cores, #sources) sources, one per thread."""
-    import oracle
-
-    cores = os.cpu_count() or 1
-    k = int(min(cores, len(srcs_all)))
-    sample = srcs_all[:k]
-    t0 = time.perf_counter()
-    far, reach, _, used = oracle.closeness(n, rp, ci, sample, nthreads=k)
-    dt = time.perf_counter() - t0
-    # component edges of the sampled sources: RMAT/G(n,m)/grid sources of one component share the numerator; recompute exactly
-    e = 0
-    lv0 = None
-    for s, r in zip(sample, reach):
-        if lv0 is None or lv0[int(s)] < 0:
-            lv0 = oracle.bfs(n, rp, ci, int(s))
-        e += component_edges(deg, lv0)
-    return {"value": e / dt / 1e9, "unit": "GTEPS", "cores": int(used), "kind": "oracle", "seconds": dt,
-            "sample": f"first {k} of the config's {len(srcs_all)} sources, one plain queue BFS per OpenMP thread"}
+    if not ok:
+        sys.exit(1)
 
 
 if __name__ == "__main__":

@@ -205,10 +205,12 @@ def make_config(name: str, shrink: int = 0):
     raise KeyError(name)
 
 
-def config_sources(name: str, rowptr: np.ndarray) -> np.ndarray:
+def config_sources(name: str, rowptr: np.ndarray, replica: int = 0) -> np.ndarray:
+    """The config's seeded sources.  replica > 0: another draw of the same size from the same population (seed
+    S_i + 1 + 1000 * replica) -- the disjoint per-rank work of a multi-GPU weak-scaling run."""
     c = CONFIGS[name]
     k = c["n_sources"]
-    srcs = pick_sources(rowptr, k, c["seed"] + 1, nonzero_degree=True) if k else np.empty(0, np.uint32)
+    srcs = pick_sources(rowptr, k, c["seed"] + 1 + 1000 * replica, nonzero_degree=True) if k else np.empty(0, np.uint32)
     if c["kind"] == "grid":  # corner vertex first (BASELINE.json config 2)
         srcs = np.concatenate([np.zeros(1, np.uint32), srcs])
     return srcs

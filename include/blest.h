@@ -15,10 +15,17 @@
  *    HOST pointers (pinned or pageable): the library detects which with cudaPointerGetAttributes and, for
  *    host outputs, copies device->host on `cuda_stream` inside the call.
  *  - Asynchrony: traversal calls enqueue on `cuda_stream` (a cudaStream_t cast to void*, NULL = legacy
- *    default stream) and return; results are valid once the stream is synchronised.  One handle owns one
- *    workspace: calls on the same handle must be stream-ordered.  Host `srcs` arrays are consumed before return.
+ *    default stream) and return without waiting for the device; results are valid once the stream is
+ *    synchronised.  One handle owns one workspace: calls on the same handle must be stream-ordered.  Host
+ *    `srcs` arrays are consumed before return (copied to a handle-owned pinned staging slot; temporaries are
+ *    stream-ordered allocations).  Because the calls do not wait, an error that only the device can see (an
+ *    internal work-queue overflow) cannot be returned by the call that caused it: it is latched in the handle,
+ *    returned by blest_last_status() and by every later traversal call on the handle until it is read there.
  *  - Graph precondition: symmetric (undirected) CSR, rows sorted ascending, column ids < n,
- *    rowptr[0] = 0, rowptr[n] = nnz < 2^32, 1 <= n <= 2^29.  Unsorted rows are always detected
+ *    rowptr[0] = 0, rowptr[n] = nnz < 2^32, 1 <= n <= 2^29 (narrower than uint32 because the kernels pack flags
+ *    beside ids: bit 31 of a vertex id in the inline heads / bottom-up lists, 5 bits beside a slice-set id in a
+ *    32-bit queue entry; the largest config has n = 2^25).  Self-loops and duplicate entries are legal and have no
+ *    effect on the result.  Unsorted rows are always detected
  *    (BLEST_EUNSORTED); symmetry and ranges are checked only when options.validate != 0.
  */
 #ifndef BLEST_H
@@ -41,7 +48,8 @@ enum {
   BLEST_ENOMEM = -5,       /* host or device allocation failed */
   BLEST_ECUDA = -6,        /* a CUDA call failed; see blest_last_cuda_error() */
   BLEST_EUNSUPPORTED = -7, /* no sm_100 device / cooperative launch unavailable */
-  BLEST_EOVERFLOW = -8     /* internal work queue overflow (should not happen; reported, never silent) */
+  BLEST_EOVERFLOW = -8     /* internal work queue overflow (should not happen with the automatic capacities; latched
+                              by the kernels, reported by blest_last_status() and by later calls, never silent) */
 };
 
 /* Input graph ("CSC of A"; symmetric here, so one CSR serves as A, A^T and Alg. 4's CSR(G^T)). */
@@ -58,7 +66,7 @@ typedef struct {
  * policy-independence tests and the ablation axes of PAPER.md Tables 4/6). */
 typedef struct {
   int reorder;     /* 0 none | 1 RCM | 2 degree-descending (BASELINE.json config 4) */
-  int builder;     /* 0 host (OpenMP) | 1 device (BVSS built by CUDA kernels) */
+  int builder;     /* 0 host (OpenMP over slice sets).  No other builder exists: any other value is BLEST_EINVAL */
   int validate;    /* 0 | 1: O(nnz log d) symmetry + range check */
   int kernel;      /* 0 auto by U_div | 1 eager (Alg. 2) | 2 lazy two-stage (Alg. 3) */
   int switching;   /* 0 auto (per-level cost model; Eq. 6 analogue) | 1 off: slice path only |
@@ -70,6 +78,17 @@ typedef struct {
   int trace;       /* 0 | 1: keep the per-level trace (always cheap; default on) */
   float eta;       /* bottom-up switch constant (Eq. 6, eta = 10 on Hopper); 0 -> library default */
   float gamma;     /* scales the slice-path cost in the per-slice-set slice-vs-CSR-edges threshold; 0 -> 1.0 */
+  int persist_l2;  /* 0 auto | 1 off.  auto: a single-source traversal of a REORDERED graph whose 4n-byte levels_out
+                      fits the device's persisting-L2 carve-out writes levels straight to original ids under a
+                      persisting access-policy window of that launch; while such handles exist the library owns
+                      cudaLimitPersistingL2CacheSize of the device (the value found is restored by the last
+                      blest_destroy).  off: levels go to an internal-id array and one gather pass ends the call. */
+  int prune_components; /* 0 on | 1 off.  on: blest_build labels the connected component of the highest-degree vertex
+                      (one host BFS, timed as info.component_seconds); a traversal whose source lies in it starts
+                      with everything outside marked visited, so no sweep examines vertices it cannot reach.
+                      Result-neutral; not part of the paper's method. */
+  uint32_t queue_capacity; /* 0 auto (exact bounds) | entries: caps the work queues / chunk list (tests of the
+                      overflow report) */
   int reserved[6]; /* [0]: switching == 5 ("scripted", tests): level l runs bottom-up iff bit min(l,31) is set;
                       [1..5]: tuning overrides of the switch cost model in 0.01 ps per unit (top-down edge, top-down
                       vertex, bottom-up vertex, bottom-up scanned neighbour, bottom-up bitmap word); 0 = default */
@@ -88,6 +107,7 @@ typedef struct {
   double mask_density;     /* nnz / n_slices (rho_c, 1..8) */
   double u_div;            /* update divergence (reading R20) */
   double reorder_seconds, build_seconds, upload_seconds;
+  double component_seconds; /* options.prune_components: host BFS labelling the hub's component (0 when off) */
   int kernel_chosen;       /* 1 eager | 2 lazy (after auto dispatch) */
   int reorder, kappa, num_sms, grid_blocks, block_threads;
   uint32_t queue_capacity; /* entries per work queue */
@@ -139,7 +159,29 @@ int blest_closeness(blest_handle_t h, const uint32_t *srcs, uint64_t n_srcs, dou
 int blest_farness(blest_handle_t h, const uint32_t *srcs, uint64_t n_srcs, uint64_t *far_out, uint32_t *reach_out,
                   void *cuda_stream);
 
+/* Multi-GPU closeness by source partition ("sources partitioned over GPUs, partial sums reduced at the
+ * end"): the target-side sums of Eq. 7 over the source range [first, first + count) only.  far_sum uint64[n],
+ * reach_sum uint32[n], DEVICE pointers, indexed by ORIGINAL vertex id: far_sum[v] = sum over the sources s of the range
+ * of d(s, v), reach_sum[v] = how many of them reach v.  Summing the arrays of disjoint ranges that cover 0..n-1 (one
+ * all-reduce) gives the farness / reach of every vertex (the graph is undirected); blest_closeness_from_sums divides. */
+int blest_farness_partial(blest_handle_t h, uint32_t first, uint32_t count, uint64_t *far_sum, uint32_t *reach_sum,
+                          void *cuda_stream);
+
+/* out[v] = (reach_sum[v] - 1) / far_sum[v] in fp64, 0.0 when far_sum[v] = 0 (Eq. 8, reading R14).  Device pointers. */
+int blest_closeness_from_sums(const uint64_t *far_sum, const uint32_t *reach_sum, uint64_t n, double *out,
+                              void *cuda_stream);
+
+/* Totals of the most recent multi-source launch, for the roofline (needs options.trace): out8[0] work-queue entries
+ * (VSS chunks) consumed by Stage 1, [1] quads they hold, [2] slices whose V_next word was probed, [3] row words updated
+ * by an atomic, [4] dirty slice sets swept by Stage 2, [5] levels, [6] source batches, [7] 0.  Synchronises the device. */
+int blest_get_ms_stats(blest_handle_t h, uint64_t *out8);
+
 int blest_get_info(blest_handle_t h, blest_info_t *info);
+
+/* Deferred status of the handle: synchronises the device, returns BLEST_EOVERFLOW if any traversal since the last
+ * call of this function overflowed an internal work queue (its results are then incomplete), else BLEST_OK, and
+ * clears the latch. */
+int blest_last_status(blest_handle_t h);
 
 /* Per-level trace of the last blest_bfs call.  Synchronises the device.  *n_levels = records available
  * (may exceed cap; only min(cap, available) are copied). */
@@ -168,6 +210,10 @@ int blest_contraction_selftest(int contraction, uint64_t *n_mismatch);
  * reports tera-ops/s (one op = one multiply-accumulate on one bit (b1) or one byte (u8)), 2 ops per MAC not applied.
  * kind: 2 = mma.sync m8n8k128 b1 and.popc | 3 = mma.sync m16n8k32 u8. */
 int blest_mma_microbench(int kind, uint32_t iters, double *tera_macs_per_s, double *milliseconds);
+
+/* L2 bandwidth microbenchmark (roofline denominator of the L2-resident multi-source path): a 16-byte-per-thread copy
+ * between two buffers of bytes/2 each, `iters` passes, in the persistent launch configuration; read + write GB/s. */
+int blest_l2_microbench(uint64_t bytes, uint32_t iters, double *gb_per_s);
 
 /* Grid-barrier latency microbenchmark: `iters` back-to-back grid barriers in the persistent launch configuration. */
 int blest_barrier_microbench(uint32_t iters, double *ns_per_barrier);

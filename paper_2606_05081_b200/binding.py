@@ -43,6 +43,7 @@ class _Options(ctypes.Structure):
     _fields_ = [("reorder", ctypes.c_int), ("builder", ctypes.c_int), ("validate", ctypes.c_int),
                 ("kernel", ctypes.c_int), ("switching", ctypes.c_int), ("contraction", ctypes.c_int),
                 ("kappa", ctypes.c_int), ("trace", ctypes.c_int), ("eta", ctypes.c_float), ("gamma", ctypes.c_float),
+                ("persist_l2", ctypes.c_int), ("prune_components", ctypes.c_int), ("queue_capacity", ctypes.c_uint32),
                 ("reserved", ctypes.c_int * 6)]
 
 
@@ -52,7 +53,7 @@ class _Info(ctypes.Structure):
                 ("bvss_bytes", ctypes.c_uint64), ("csr_bytes", ctypes.c_uint64), ("workspace_bytes", ctypes.c_uint64),
                 ("mask_density", ctypes.c_double), ("u_div", ctypes.c_double), ("reorder_seconds", ctypes.c_double),
                 ("build_seconds", ctypes.c_double), ("upload_seconds", ctypes.c_double),
-                ("kernel_chosen", ctypes.c_int), ("reorder", ctypes.c_int), ("kappa", ctypes.c_int),
+                ("component_seconds", ctypes.c_double), ("kernel_chosen", ctypes.c_int), ("reorder", ctypes.c_int), ("kappa", ctypes.c_int),
                 ("num_sms", ctypes.c_int), ("grid_blocks", ctypes.c_int), ("block_threads", ctypes.c_int),
                 ("queue_capacity", ctypes.c_uint32), ("n_sweep_words", ctypes.c_uint32)]
 
@@ -69,7 +70,8 @@ TRACE_DTYPE = np.dtype([("level", "<u4"), ("mode", "<u4"), ("q_entries", "<u4"),
                         ("t_ns", "<u8"), ("t_stage1_ns", "<u8")])
 
 EXPORTS = ["blest_build", "blest_preprocess_host", "blest_configure", "blest_get_call_stats", "blest_bfs", "blest_msbfs", "blest_closeness", "blest_farness",
-           "blest_get_info", "blest_get_trace", "blest_get_array", "blest_get_vi", "blest_contraction_selftest",
+           "blest_get_info", "blest_last_status", "blest_farness_partial", "blest_closeness_from_sums", "blest_get_ms_stats",
+           "blest_l2_microbench", "blest_get_trace", "blest_get_array", "blest_get_vi", "blest_contraction_selftest",
            "blest_mma_microbench", "blest_barrier_microbench", "blest_destroy", "blest_strerror",
            "blest_last_cuda_error"]
 
@@ -93,6 +95,11 @@ def load(build_if_missing: bool = True):
     L.blest_closeness.argtypes = [vp, vp, u64, vp, vp]
     L.blest_farness.argtypes = [vp, vp, u64, vp, vp, vp]
     L.blest_get_info.argtypes = [vp, ctypes.POINTER(_Info)]
+    L.blest_last_status.argtypes = [vp]
+    L.blest_farness_partial.argtypes = [vp, u32, u32, vp, vp, vp]
+    L.blest_closeness_from_sums.argtypes = [vp, vp, u64, vp, vp]
+    L.blest_get_ms_stats.argtypes = [vp, ctypes.POINTER(u64)]
+    L.blest_l2_microbench.argtypes = [u64, u32, ctypes.POINTER(ctypes.c_double)]
     L.blest_get_trace.argtypes = [vp, vp, u32, ctypes.POINTER(u32)]
     L.blest_get_call_stats.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
     L.blest_get_array.argtypes = [vp, i32, vp, u64]
@@ -141,7 +148,8 @@ def _stream(stream):
 
 
 def _options(reorder="none", builder=0, validate=False, kernel="auto", switching="auto", contraction="auto", kappa=64,
-             trace=True, eta=0.0, gamma=0.0, bu_mask=0, costs=None) -> _Options:
+             trace=True, eta=0.0, gamma=0.0, bu_mask=0, costs=None, persist_l2=True, prune_components=True,
+             queue_capacity=0) -> _Options:
     o = _Options()
     o.reorder = REORDER[reorder] if isinstance(reorder, str) else int(reorder)
     o.builder = int(builder)
@@ -153,6 +161,9 @@ def _options(reorder="none", builder=0, validate=False, kernel="auto", switching
     o.trace = int(bool(trace))
     o.eta = float(eta)
     o.gamma = float(gamma)
+    o.persist_l2 = 0 if persist_l2 else 1
+    o.prune_components = 0 if prune_components else 1
+    o.queue_capacity = int(queue_capacity)
     o.reserved[0] = int(bu_mask)
     for k, c in enumerate(costs or ()):  # switch cost model overrides, ps per unit (tuning only): td_edge, td_vertex,
         o.reserved[1 + k] = int(round(100 * float(c)))  # bu_vertex, bu_scan, bu_word
@@ -163,7 +174,7 @@ def _options(reorder="none", builder=0, validate=False, kernel="auto", switching
 class Info:
     n: int; nnz: int; n_slice_sets: int; n_vss: int; n_slices: int; n_quads: int
     bvss_bytes: int; csr_bytes: int; workspace_bytes: int; mask_density: float; u_div: float
-    reorder_seconds: float; build_seconds: float; upload_seconds: float
+    reorder_seconds: float; build_seconds: float; upload_seconds: float; component_seconds: float
     kernel_chosen: int; reorder: int; kappa: int; num_sms: int; grid_blocks: int; block_threads: int
     queue_capacity: int; n_sweep_words: int
 
@@ -244,11 +255,28 @@ class Graph:
         _check(load().blest_farness(self._h, sp, k, _ptr(far_out), _ptr(reach_out), _stream(stream)), "blest_farness")
         return far_out, reach_out
 
+    def farness_partial(self, first: int, count: int, far_sum, reach_sum, stream=None):
+        """blest_farness_partial: target-side sums over sources [first, first+count) (device tensors, original ids)."""
+        _check(load().blest_farness_partial(self._h, int(first), int(count), _ptr(far_sum), _ptr(reach_sum), _stream(stream)),
+               "blest_farness_partial")
+        return far_sum, reach_sum
+
+    def ms_stats(self) -> dict:
+        """Totals of the last multi-source launch (blest_get_ms_stats)."""
+        buf = (ctypes.c_uint64 * 8)()
+        _check(load().blest_get_ms_stats(self._h, buf), "blest_get_ms_stats")
+        keys = ("entries", "quads", "probes", "fresh", "dirty_sets", "levels", "batches")
+        return {k: int(buf[i]) for i, k in enumerate(keys)}
+
     # -- introspection
     def info(self) -> Info:
         i = _Info()
         _check(load().blest_get_info(self._h, ctypes.byref(i)), "blest_get_info")
         return Info(**{f[0]: getattr(i, f[0]) for f in _Info._fields_})
+
+    def last_status(self) -> int:
+        """blest_last_status: synchronises, returns and clears the handle's deferred status (OK or EOVERFLOW)."""
+        return int(load().blest_last_status(self._h))
 
     def call_stats(self):
         """(init_ns, levels_ns) of the last bfs call on the lazy kernel."""
@@ -294,6 +322,20 @@ def mma_microbench(kind, iters: int = 4096):
     t, ms = ctypes.c_double(0), ctypes.c_double(0)
     _check(load().blest_mma_microbench(k, iters, ctypes.byref(t), ctypes.byref(ms)), "blest_mma_microbench")
     return t.value, ms.value
+
+
+def closeness_from_sums(far_sum, reach_sum, out, stream=None):
+    n = int(out.numel()) if hasattr(out, "numel") else int(out.size)
+    _check(load().blest_closeness_from_sums(_ptr(far_sum), _ptr(reach_sum), n, _ptr(out), _stream(stream)),
+           "blest_closeness_from_sums")
+    return out
+
+
+def l2_microbench(nbytes: int = 48 << 20, iters: int = 50) -> float:
+    """Read + write GB/s of an L2-resident copy in the persistent launch configuration."""
+    g = ctypes.c_double(0)
+    _check(load().blest_l2_microbench(int(nbytes), int(iters), ctypes.byref(g)), "blest_l2_microbench")
+    return g.value
 
 
 def barrier_microbench(iters: int = 2000) -> float:

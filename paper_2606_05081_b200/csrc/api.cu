@@ -3,6 +3,8 @@
 #include <chrono>
 #include <cstdio>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -13,6 +15,7 @@ namespace blest {
 cudaError_t run_contraction_selftest(int contraction, unsigned long long* dMismatch);
 cudaError_t run_mma_peak(int kind, uint32_t iters, int blocks, int* dSink, double* macsPerLaunch);
 cudaError_t run_barrier_bench(unsigned int* dBar, uint32_t iters, int blocks, unsigned long long* dNs);
+cudaError_t run_l2_copy(const uint4* src, uint4* dst, uint64_t n16, uint32_t iters, int blocks);
 }  // namespace blest
 
 using namespace blest;
@@ -65,15 +68,24 @@ struct blest_graph {
   uint32_t *dV = nullptr, *dF[3] = {nullptr, nullptr, nullptr}, *dWL[2] = {nullptr, nullptr};
   uint4* dChunks = nullptr;
   uint2* dQ[2] = {nullptr, nullptr};
-  Ctrl* dCtrl = nullptr;
+  Ctrl* dCtrl = nullptr;      // eager / multi-source kernels: zeroed by a memset node before every launch
+  Ctrl* dCtrlLazy = nullptr;  // lazy kernel: zeroed once here, self-resetting afterwards (no memset per call)
+  Ctrl* lastCtrl = nullptr;   // control block of the most recent traversal (blest_get_trace / blest_get_call_stats)
+  unsigned int* hStatus = nullptr;  // host-mapped latch: a kernel that overflows a work queue stores 1 here
+  int device = 0;
+  bool persistRef = false;    // this handle holds a reference on the device's persisting-L2 state
   blest_level_trace_t* dTrace = nullptr;
   int32_t *dL = nullptr, *dStamp = nullptr, *dOut = nullptr;
-  // multi-source workspace (allocated on first use for the current kappa)
-  int msKappa = 0;
+  // multi-source workspace: grow-only (sized for the widest kappa used so far; a wider kappa frees and re-allocates)
+  uint64_t msWords = 0;
   uint32_t *dMsF = nullptr, *dMsVc = nullptr, *dMsVn = nullptr;
+  // pinned staging slots for host `srcs` arrays (consumed before the call returns; recycled once their copy has run)
+  struct StageSlot { void* host = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; };
+  std::vector<StageSlot> stage;
   uint8_t* dDirty = nullptr;
   unsigned long long* dFarT = nullptr;
   uint32_t* dReachT = nullptr;
+  unsigned long long* dMsStats = nullptr;  // [8] totals of the last multi-source launch (blest_get_ms_stats)
   uint64_t wsBytes = 0;
   std::vector<void*> allocs;
 };
@@ -107,7 +119,8 @@ static void normalise_options(blest_options_t& o) {
 }
 
 static int check_options(const blest_options_t& o) {
-  if (o.reorder < 0 || o.reorder > 2 || o.builder < 0 || o.builder > 1) return BLEST_EINVAL;
+  if (o.reorder < 0 || o.reorder > 2 || o.builder != 0) return BLEST_EINVAL;
+  if (o.persist_l2 < 0 || o.persist_l2 > 1 || o.prune_components < 0 || o.prune_components > 1) return BLEST_EINVAL;
   if (o.kernel < 0 || o.kernel > 2 || o.switching < 0 || o.switching > 5) return BLEST_EINVAL;
   if (o.contraction < 0 || o.contraction > 3) return BLEST_EINVAL;
   if (o.kappa != 0 && o.kappa != 32 && o.kappa != 64 && o.kappa != 128 && o.kappa != 256) return BLEST_EINVAL;
@@ -149,35 +162,69 @@ static int upload_pop_thresholds(blest_graph* g) {
   return BLEST_OK;
 }
 
-// Persisting-L2 set-aside (device-wide limit): only while a reordered graph's single-source traversals use it; an unused
-// set-aside just shrinks the L2 for everything else (measured: 3x slower bottom-up levels), so every other path sets 0.
-static int g_persistMax() {
-  static int v = -1;
-  if (v < 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxPersistingL2CacheSize, dev) != cudaSuccess) v = 0;
+// Persisting-L2 set-aside.  cudaLimitPersistingL2CacheSize is a DEVICE-wide limit, so it is managed per device, under a
+// lock, and only while handles that use it exist (options.persist_l2 = auto on a reordered graph): the first such handle
+// records the limit it found, the last blest_destroy restores it.  While the library owns it, the set-aside is switched on
+// for the lazy single-source traversals that put a window over levels_out and off for every other path (an unused
+// set-aside just shrinks the L2 for everything else: measured 3x slower bottom-up levels).
+struct PersistState {
+  int refs = 0;
+  size_t original = 0, current = 0;
+  int maxPersist = -1, maxWindow = -1;
+};
+static std::mutex g_persistMutex;
+static std::map<int, PersistState> g_persist;
+
+static PersistState& persist_state_locked(int dev) {
+  PersistState& ps = g_persist[dev];
+  if (ps.maxPersist < 0) {
+    if (cudaDeviceGetAttribute(&ps.maxPersist, cudaDevAttrMaxPersistingL2CacheSize, dev) != cudaSuccess) ps.maxPersist = 0;
+    if (cudaDeviceGetAttribute(&ps.maxWindow, cudaDevAttrMaxAccessPolicyWindowSize, dev) != cudaSuccess) ps.maxWindow = 0;
     cudaGetLastError();
   }
-  return v;
+  return ps;
 }
-static int g_windowMax() {
-  static int v = -1;
-  if (v < 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxAccessPolicyWindowSize, dev) != cudaSuccess) v = 0;
+static void persist_acquire(blest_graph* g) {
+  std::lock_guard<std::mutex> lk(g_persistMutex);
+  PersistState& ps = persist_state_locked(g->device);
+  if (ps.refs++ == 0) {
+    if (cudaDeviceGetLimit(&ps.original, cudaLimitPersistingL2CacheSize) != cudaSuccess) ps.original = 0;
     cudaGetLastError();
+    ps.current = ps.original;
   }
-  return v;
+  g->persistRef = true;
 }
-static void set_persisting_l2(size_t bytes) {
-  static size_t current = 0;
-  if (bytes == current) return;
+static void persist_set_locked(PersistState& ps, size_t bytes) {
+  if (bytes == ps.current) return;
   if (bytes == 0) cudaCtxResetPersistingL2Cache();
   cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, bytes);
   cudaGetLastError();
-  current = bytes;
+  ps.current = bytes;
+}
+static void persist_release(blest_graph* g) {
+  if (!g->persistRef) return;
+  std::lock_guard<std::mutex> lk(g_persistMutex);
+  PersistState& ps = persist_state_locked(g->device);
+  if (--ps.refs == 0) persist_set_locked(ps, ps.original);
+  g->persistRef = false;
+}
+// Called by every traversal of a handle that holds a reference: bytes > 0 switches the set-aside on (capped at the
+// device maximum), 0 switches it off.  Returns the bytes in force.
+static size_t persist_use(blest_graph* g, size_t bytes) {
+  if (!g->persistRef) return 0;
+  std::lock_guard<std::mutex> lk(g_persistMutex);
+  PersistState& ps = persist_state_locked(g->device);
+  persist_set_locked(ps, bytes ? (size_t)ps.maxPersist : 0);
+  return ps.current;
+}
+static bool persist_fits(blest_graph* g, size_t bytes) {
+  std::lock_guard<std::mutex> lk(g_persistMutex);
+  PersistState& ps = persist_state_locked(g->device);
+  return bytes <= (size_t)ps.maxPersist && bytes <= (size_t)ps.maxWindow;
+}
+static size_t persist_max(blest_graph* g) {
+  std::lock_guard<std::mutex> lk(g_persistMutex);
+  return (size_t)persist_state_locked(g->device).maxPersist;
 }
 
 extern "C" {
@@ -203,8 +250,17 @@ uint64_t blest_get_vi(uint64_t u, uint64_t rho) { return (u % SIGMA) * rho + u /
 
 void blest_destroy(blest_handle_t h) {
   if (!h) return;
-  if (!h->hostOnly) set_persisting_l2(0);
+  if (!h->hostOnly) {
+    cudaDeviceSynchronize();  // enqueued work may still use the workspace
+    cudaGetLastError();
+    persist_release(h);
+  }
   for (void* p : h->allocs) cudaFree(p);
+  for (auto& sl : h->stage) {
+    if (sl.ev) cudaEventDestroy(sl.ev);
+    if (sl.host) cudaFreeHost(sl.host);
+  }
+  if (h->hStatus) cudaFreeHost(h->hStatus);
   delete h;
 }
 
@@ -217,12 +273,11 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
   if (rc) return rc;
   normalise_options(opt);
   if (csr->n == 0 || csr->n > (1u << 29) || csr->nnz > 0xFFFFFFFFull) return BLEST_ERANGE;
-  if (opt.builder == 1) return BLEST_EUNSUPPORTED;  // device builder: not in this round
   if (hostOnly && csr->on_device) return BLEST_EINVAL;
 
-  int sms = 0;
+  int sms = 0, dev = 0;
   if (!hostOnly) {
-    int dev = 0, major = 0, coop = 0;
+    int major = 0, coop = 0;
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
     CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
@@ -233,6 +288,7 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
   blest_graph* g = new (std::nothrow) blest_graph();
   if (!g) return BLEST_ENOMEM;
   g->hostOnly = hostOnly;
+  g->device = dev;
   struct Guard { blest_graph* g; ~Guard() { if (g) blest_destroy(g); } } guard{g};
 
   try {
@@ -297,7 +353,8 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
       // Connected component of the highest-degree vertex (level-synchronous host BFS, OpenMP over the frontier).  A
       // traversal from a source inside it can never leave it, so the lazy kernel starts with everything outside marked
       // visited: no sweep ever examines those vertices, and the traversal ends as soon as the component is exhausted.
-      if (!hostOnly && any) {
+      if (!hostOnly && any && opt.prune_components == 0) {
+        const double tc0 = now_s();
         uint32_t hub = 0, best = 0;
         for (uint32_t u = 0; u < g->n; ++u) {
           const uint32_t d = gcsr->rowptr[u + 1] - gcsr->rowptr[u];
@@ -332,6 +389,7 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
           outside += (uint32_t)__builtin_popcount(~g->hubComp[w] & valid);
         }
         g->nOutsideInSweep = outside;
+        g->info.component_seconds = now_s() - tc0;
       }
     }
     // scale-free-like test in the spirit of PAPER.md:199 (fn. 2: the top 1 % of the vertices hold a large share of the
@@ -420,6 +478,7 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
       const uint64_t qcap64 = (uint64_t)g->Nv + g->n + g->nnz / TD_CHUNK + 1024;
       if (qcap64 > 0xFFFFFFF0ull) return BLEST_ERANGE;
       g->qcap = (uint32_t)qcap64;
+      if (opt.queue_capacity) g->qcap = std::min(g->qcap, std::max(opt.queue_capacity, 1u));
       if ((rc = dev_alloc(g, &g->dV, (uint64_t)g->nwords + 16, true))) return rc;
       for (int k = 0; k < 3; ++k)
         if ((rc = dev_alloc(g, &g->dF[k], (uint64_t)g->nwords + 16, true))) return rc;
@@ -429,10 +488,17 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
       // (with one word per warp the thresholds are lower, but then there are at most 36 segments per warp of the grid)
       g->chunkCap = (uint32_t)(g->nnz / CHUNK_EDGES + g->nQuads / CHUNK_QUADS + g->nnz / BIG_EDGES + g->nQuads / BIG_QUADS + 16 +
                                36ull * 32ull * 1024ull);
-      if ((rc = dev_alloc(g, &g->dChunks, g->chunkCap))) return rc;
-      if ((rc = dev_alloc(g, &g->dQ[0], g->qcap))) return rc;
-      if ((rc = dev_alloc(g, &g->dQ[1], g->qcap))) return rc;
+      if (opt.queue_capacity) g->chunkCap = std::min(g->chunkCap, std::max(opt.queue_capacity, 1u));
+      // the lists are zeroed: after an overflow (options.queue_capacity) a consumer may read an entry that was never
+      // written, and an all-zero entry is an empty / in-range work item
+      if ((rc = dev_alloc(g, &g->dChunks, g->chunkCap, true))) return rc;
+      if ((rc = dev_alloc(g, &g->dQ[0], g->qcap, true))) return rc;
+      if ((rc = dev_alloc(g, &g->dQ[1], g->qcap, true))) return rc;
       if ((rc = dev_alloc(g, &g->dCtrl, 1, true))) return rc;
+      if ((rc = dev_alloc(g, &g->dCtrlLazy, 1, true))) return rc;
+      CK(cudaHostAlloc((void**)&g->hStatus, sizeof(unsigned int), cudaHostAllocMapped));
+      *g->hStatus = 0;
+      if (g->hasPerm && opt.persist_l2 == 0) persist_acquire(g);
       if ((rc = dev_alloc(g, &g->dTrace, TRACE_CAP, true))) return rc;
       if ((rc = dev_alloc(g, &g->dStamp, g->Ns))) return rc;
       if ((rc = dev_alloc(g, &g->dOut, g->n))) return rc;
@@ -481,11 +547,17 @@ int blest_configure(blest_handle_t h, const blest_options_t* optIn) {
   o.reorder = h->opt.reorder;
   o.builder = h->opt.builder;
   o.validate = h->opt.validate;
+  o.prune_components = h->opt.prune_components;
+  o.queue_capacity = h->opt.queue_capacity;
   int rc = check_options(o);
   if (rc) return rc;
   normalise_options(o);
   const bool gammaChanged = o.gamma != h->opt.gamma;
   h->opt = o;
+  if (!h->hostOnly && h->hasPerm) {
+    if (o.persist_l2 == 0 && !h->persistRef) persist_acquire(h);
+    if (o.persist_l2 == 1 && h->persistRef) persist_release(h);
+  }
   if (gammaChanged && !h->hostOnly) return upload_pop_thresholds(h);
   return BLEST_OK;
 }
@@ -504,10 +576,25 @@ int blest_get_info(blest_handle_t h, blest_info_t* info) {
   return BLEST_OK;
 }
 
+// Deferred device-side errors (include/blest.h "Asynchrony"): latched by the kernels in a host-mapped word.
+static int pending_status(blest_graph* h) {
+  return (h->hStatus && *(volatile unsigned int*)h->hStatus) ? BLEST_EOVERFLOW : BLEST_OK;
+}
+
+int blest_last_status(blest_handle_t h) {
+  if (!h) return BLEST_EINVAL;
+  if (h->hostOnly) return BLEST_OK;
+  CK(cudaDeviceSynchronize());
+  const int rc = pending_status(h);
+  *(volatile unsigned int*)h->hStatus = 0;
+  return rc;
+}
+
 int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_stream) {
   if (!h || !levels_out) return BLEST_EINVAL;
   if (h->hostOnly) return BLEST_EUNSUPPORTED;
   if (src >= h->n) return BLEST_EINVAL;
+  if (int rc = pending_status(h)) return rc;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const bool devOut = is_device_ptr(levels_out);
   BfsParams p{};
@@ -532,7 +619,7 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
   p.out = devOut ? levels_out : h->dOut;
   p.L = h->hasPerm ? h->dL : p.out;
   p.stamp = h->dStamp;
-  p.ctrl = h->dCtrl;
+  p.hostStatus = h->hStatus;
   p.trace = h->opt.trace == 0 || h->opt.trace == 1 ? h->dTrace : nullptr;
   p.traceCap = TRACE_CAP;
   p.src = h->hasPerm ? h->perm[src] : src;
@@ -551,27 +638,31 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
   p.buMask = (uint32_t)h->opt.reserved[0];
   p.eta = h->opt.eta;
   p.gamma = h->opt.gamma;
-  CK(cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st));
-  if ((h->isoBits[p.src >> 5] >> (p.src & 31u)) & 1u) CK(launch_isolated_source(p.out, h->n, src, st));  // nothing to traverse
-  else if (resolved_kernel(h) == 1) {
-    set_persisting_l2(0);
+  if ((h->isoBits[p.src >> 5] >> (p.src & 31u)) & 1u) {
+    h->lastCtrl = nullptr;
+    CK(launch_isolated_source(p.out, h->n, src, st));  // nothing to traverse
+  } else if (resolved_kernel(h) == 1) {
+    persist_use(h, 0);
+    p.ctrl = h->dCtrl;
+    h->lastCtrl = h->dCtrl;
+    CK(cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st));
     CK(launch_bfs_eager(p, h->gridEager, st));
-  }
-  else {
+  } else {
     // levels_out is written once per discovered vertex at a scattered (original-id) position when the graph was
     // reordered: keep its lines in L2 for the duration of the call (persisting access-policy window of the launch),
     // so that those 4-byte writes merge there instead of each costing DRAM a sector.  Measured on C4: -5..10 % per BFS.
     const size_t bytes = (size_t)h->n * 4;
-    static const bool envOff = getenv("BLEST_PERSIST") && atoi(getenv("BLEST_PERSIST")) == 0;
-    const bool usePersist = !envOff && h->hasPerm && bytes <= (size_t)g_persistMax() && bytes <= (size_t)g_windowMax();
+    const bool usePersist = h->persistRef && persist_fits(h, bytes);
     // reordered graph: levels scattered straight into levels_out when L2 can hold it, else internal array + gather pass
     p.gather = h->hasPerm && !usePersist;
     p.lvl = p.gather ? h->dL : p.out;
     p.ipermW = (h->hasPerm && !p.gather) ? h->dIperm : nullptr;
     p.srcLvl = p.gather ? p.src : src;
-    set_persisting_l2(usePersist ? (size_t)g_persistMax() : 0);
+    p.ctrl = h->dCtrlLazy;  // self-resetting: no memset node before the launch
+    h->lastCtrl = h->dCtrlLazy;
+    persist_use(h, usePersist ? bytes : 0);
     const cudaError_t le = launch_bfs_lazy(p, h->gridLazy, st, usePersist ? (const void*)p.out : nullptr, usePersist ? bytes : 0,
-                                           usePersist ? (float)std::min(1.0, (double)g_persistMax() / (double)bytes) : 0.f);
+                                           usePersist ? (float)std::min(1.0, (double)persist_max(h) / (double)bytes) : 0.f);
     CK(le);
   }
   if (!devOut) CK(cudaMemcpyAsync(levels_out, h->dOut, (size_t)h->n * 4, cudaMemcpyDeviceToHost, st));
@@ -582,8 +673,8 @@ int blest_get_trace(blest_handle_t h, blest_level_trace_t* buf, uint32_t cap, ui
   if (!h || !n_levels) return BLEST_EINVAL;
   if (h->hostOnly) return BLEST_EUNSUPPORTED;
   CK(cudaDeviceSynchronize());
-  Ctrl c;
-  CK(cudaMemcpy(&c, h->dCtrl, sizeof(Ctrl), cudaMemcpyDeviceToHost));
+  Ctrl c{};
+  if (h->lastCtrl) CK(cudaMemcpy(&c, h->lastCtrl, sizeof(Ctrl), cudaMemcpyDeviceToHost));
   *n_levels = c.nlevels;
   const uint32_t k = std::min(std::min(cap, c.nlevels), TRACE_CAP);
   if (buf && k) CK(cudaMemcpy(buf, h->dTrace, (size_t)k * sizeof(blest_level_trace_t), cudaMemcpyDeviceToHost));
@@ -594,8 +685,8 @@ int blest_get_call_stats(blest_handle_t h, uint64_t* init_ns, uint64_t* levels_n
   if (!h) return BLEST_EINVAL;
   if (h->hostOnly) return BLEST_EUNSUPPORTED;
   CK(cudaDeviceSynchronize());
-  Ctrl c;
-  CK(cudaMemcpy(&c, h->dCtrl, sizeof(Ctrl), cudaMemcpyDeviceToHost));
+  Ctrl c{};
+  if (h->lastCtrl) CK(cudaMemcpy(&c, h->lastCtrl, sizeof(Ctrl), cudaMemcpyDeviceToHost));
   if (init_ns) *init_ns = c.tInit;
   if (levels_ns) {
     *levels_ns = 0;
@@ -609,19 +700,32 @@ int blest_get_call_stats(blest_handle_t h, uint64_t* init_ns, uint64_t* levels_n
 }
 
 static int ensure_ms_workspace(blest_graph* g) {
-  set_persisting_l2(0);  // the multi-source state wants the whole L2
-  const int kappa = g->opt.kappa;
-  if (g->msKappa == kappa) return BLEST_OK;
+  persist_use(g, 0);  // the multi-source state wants the whole L2
+  const uint64_t words = (uint64_t)g->rho * 8u * (g->opt.kappa / 32) + 4;
   int rc;
-  const uint64_t words = (uint64_t)g->rho * 8u * (kappa / 32) + 4;
-  // (re)allocation for a different kappa simply adds buffers; the old ones are freed with the handle
-  if ((rc = dev_alloc(g, &g->dMsF, words, true))) return rc;
-  if ((rc = dev_alloc(g, &g->dMsVc, words, true))) return rc;
-  if ((rc = dev_alloc(g, &g->dMsVn, words, true))) return rc;
+  if (words > g->msWords) {
+    // grow-only: a wider kappa than any used before replaces the three state arrays (the old ones may still be in use
+    // by enqueued work, hence the synchronisation -- this happens at most three times in a handle's life)
+    if (g->dMsF) {
+      CK(cudaDeviceSynchronize());
+      for (uint32_t* old : {g->dMsF, g->dMsVc, g->dMsVn}) {
+        auto it = std::find(g->allocs.begin(), g->allocs.end(), (void*)old);
+        if (it != g->allocs.end()) g->allocs.erase(it);
+        cudaFree(old);
+      }
+      g->wsBytes -= 3 * ((g->msWords * 4 + 15) & ~15ull);
+      g->dMsF = g->dMsVc = g->dMsVn = nullptr;
+      g->msWords = 0;
+    }
+    if ((rc = dev_alloc(g, &g->dMsF, words, true))) return rc;
+    if ((rc = dev_alloc(g, &g->dMsVc, words, true))) return rc;
+    if ((rc = dev_alloc(g, &g->dMsVn, words, true))) return rc;
+    g->msWords = words;
+  }
   if (!g->dDirty && (rc = dev_alloc(g, &g->dDirty, (uint64_t)g->Ns + 16, true))) return rc;
   if (!g->dFarT && (rc = dev_alloc(g, &g->dFarT, (uint64_t)g->rho * 8u, true))) return rc;
   if (!g->dReachT && (rc = dev_alloc(g, &g->dReachT, (uint64_t)g->rho * 8u, true))) return rc;
-  g->msKappa = kappa;
+  if (!g->dMsStats && (rc = dev_alloc(g, &g->dMsStats, 8, true))) return rc;
   return BLEST_OK;
 }
 
@@ -633,7 +737,62 @@ static void fill_ms_params(blest_graph* h, MsParams& p) {
   p.F = h->dMsF; p.Vc = h->dMsVc; p.Vn = h->dMsVn; p.dirty = h->dDirty;
   p.Q[0] = h->dQ[0]; p.Q[1] = h->dQ[1];
   p.ctrl = h->dCtrl;
+  p.hostStatus = h->hStatus;
   p.kappa = h->opt.kappa;
+  p.stats = h->opt.trace ? h->dMsStats : nullptr;
+}
+
+// Stream-ordered temporaries of one multi-source call: device buffers from the stream's memory pool
+// (cudaMallocAsync / cudaFreeAsync: no host block), the caller's `srcs` copied through a pinned staging slot.
+struct MsTemps {
+  cudaStream_t st;
+  std::vector<void*> dev;
+  cudaError_t alloc(void** p, size_t bytes) {
+    cudaError_t e = cudaMallocAsync(p, std::max<size_t>(bytes, 16), st);
+    if (e == cudaSuccess) dev.push_back(*p);
+    return e;
+  }
+  void release() {
+    for (void* p : dev) cudaFreeAsync(p, st);
+    dev.clear();
+  }
+};
+
+// Copy `count` source ids to the device without blocking: host -> pinned slot (now), pinned -> device (on the stream).
+// A slot is reused once the copy that read it has executed (event query); a new one is made when none is free.
+static cudaError_t stage_srcs(blest_graph* h, const uint32_t* srcs, uint64_t count, uint32_t* dDst, cudaStream_t st) {
+  const size_t bytes = (size_t)count * 4;
+  blest_graph::StageSlot* slot = nullptr;
+  for (auto& sl : h->stage)
+    if (sl.cap >= bytes && cudaEventQuery(sl.ev) == cudaSuccess) { slot = &sl; break; }
+  cudaGetLastError();  // cudaErrorNotReady of a busy slot is not an error
+  if (!slot) {
+    if (h->stage.size() >= 16) {  // bounded: wait for the oldest copy instead of growing without limit
+      blest_graph::StageSlot old = h->stage.front();
+      h->stage.erase(h->stage.begin());
+      cudaEventSynchronize(old.ev);
+      cudaEventDestroy(old.ev);
+      cudaFreeHost(old.host);
+    }
+    blest_graph::StageSlot sl;
+    sl.cap = std::max<size_t>(bytes, 4096);
+    cudaError_t e = cudaHostAlloc(&sl.host, sl.cap, cudaHostAllocDefault);
+    if (e != cudaSuccess) return e;
+    e = cudaEventCreateWithFlags(&sl.ev, cudaEventDisableTiming);
+    if (e != cudaSuccess) { cudaFreeHost(sl.host); return e; }
+    h->stage.push_back(sl);
+    slot = &h->stage.back();
+  }
+  std::memcpy(slot->host, srcs, bytes);
+  cudaError_t e = cudaMemcpyAsync(dDst, slot->host, bytes, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = cudaEventRecord(slot->ev, st);
+  return e;
+}
+
+static int ms_fail(cudaError_t e) {
+  g_lastCuda = (int)e;
+  cudaGetLastError();
+  return e == cudaErrorMemoryAllocation ? BLEST_ENOMEM : BLEST_ECUDA;
 }
 
 int blest_msbfs(blest_handle_t h, const uint32_t* srcs, uint32_t k, int32_t* levels_out, void* cuda_stream) {
@@ -641,32 +800,30 @@ int blest_msbfs(blest_handle_t h, const uint32_t* srcs, uint32_t k, int32_t* lev
   if (h->hostOnly) return BLEST_EUNSUPPORTED;
   for (uint32_t i = 0; i < k; ++i)
     if (srcs[i] >= h->n) return BLEST_EINVAL;
+  if (int rc = pending_status(h)) return rc;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int rc = ensure_ms_workspace(h);
   if (rc) return rc;
   const bool devOut = is_device_ptr(levels_out);
+  MsTemps tmp{st, {}};
   uint32_t* dSrcs = nullptr;
   int32_t* dLevels = nullptr;
-  CK(cudaMalloc((void**)&dSrcs, (size_t)k * 4));
-  if (!devOut) {
-    cudaError_t e = cudaMalloc((void**)&dLevels, (size_t)k * h->n * 4);
-    if (e != cudaSuccess) { cudaFree(dSrcs); g_lastCuda = (int)e; cudaGetLastError(); return BLEST_ENOMEM; }
-  }
-  auto cleanup = [&]() { cudaFree(dSrcs); if (dLevels) cudaFree(dLevels); };
-  cudaError_t e = cudaMemcpyAsync(dSrcs, srcs, (size_t)k * 4, cudaMemcpyHostToDevice, st);
+  cudaError_t e = tmp.alloc((void**)&dSrcs, (size_t)k * 4);
+  if (e == cudaSuccess && !devOut) e = tmp.alloc((void**)&dLevels, (size_t)k * h->n * 4);
+  if (e == cudaSuccess) e = stage_srcs(h, srcs, k, dSrcs, st);
   MsParams p{};
   fill_ms_params(h, p);
   p.srcs = dSrcs;
   p.nsrcs = k;
   p.levels = devOut ? levels_out : dLevels;
+  h->lastCtrl = h->dCtrl;
   if (e == cudaSuccess) e = cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->dMsStats, 0, 8 * sizeof(unsigned long long), st);
   if (e == cudaSuccess) e = launch_msbfs(p, h->gridMs, st);
   if (e == cudaSuccess && !devOut)
     e = cudaMemcpyAsync(levels_out, dLevels, (size_t)k * h->n * 4, cudaMemcpyDeviceToHost, st);
-  // the temporaries (and the host srcs array) must outlive the enqueued work: this call synchronises the stream
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  cleanup();
-  if (e != cudaSuccess) { g_lastCuda = (int)e; cudaGetLastError(); return BLEST_ECUDA; }
+  tmp.release();  // stream-ordered: the buffers live until the work enqueued above has run
+  if (e != cudaSuccess) return ms_fail(e);
   return BLEST_OK;
 }
 
@@ -679,6 +836,7 @@ static int closeness_impl(blest_handle_t h, const uint32_t* srcs, uint64_t n_src
   if (srcs)
     for (uint64_t i = 0; i < n_srcs; ++i)
       if (srcs[i] >= h->n) return BLEST_EINVAL;
+  if (int rc = pending_status(h)) return rc;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int rc = ensure_ms_workspace(h);
   if (rc) return rc;
@@ -686,23 +844,17 @@ static int closeness_impl(blest_handle_t h, const uint32_t* srcs, uint64_t n_src
   unsigned long long *dFarS = nullptr, *dFarO = nullptr;
   uint32_t *dReachS = nullptr, *dReachO = nullptr;
   double* dCc = nullptr;
-  std::vector<void*> tmp;
-  auto talloc = [&](void** p, size_t bytes) -> cudaError_t {
-    cudaError_t e = cudaMalloc(p, std::max<size_t>(bytes, 16));
-    if (e == cudaSuccess) tmp.push_back(*p);
-    return e;
-  };
-  auto cleanup = [&]() { for (void* p : tmp) cudaFree(p); };
+  MsTemps tmp{st, {}};
   cudaError_t e = cudaSuccess;
   const bool ccDev = cc && is_device_ptr(cc), farDev = farOut && is_device_ptr(farOut), reachDev = reachOut && is_device_ptr(reachOut);
   MsParams p{};
   fill_ms_params(h, p);
   p.nsrcs = n_srcs;
   if (srcs) {  // arbitrary subset: per-source counts (reading R13)
-    e = talloc((void**)&dSrcs, n_srcs * 4);
-    if (e == cudaSuccess) e = talloc((void**)&dFarS, n_srcs * 8);
-    if (e == cudaSuccess) e = talloc((void**)&dReachS, n_srcs * 4);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(dSrcs, srcs, n_srcs * 4, cudaMemcpyHostToDevice, st);
+    e = tmp.alloc((void**)&dSrcs, n_srcs * 4);
+    if (e == cudaSuccess) e = tmp.alloc((void**)&dFarS, n_srcs * 8);
+    if (e == cudaSuccess) e = tmp.alloc((void**)&dReachS, n_srcs * 4);
+    if (e == cudaSuccess) e = stage_srcs(h, srcs, n_srcs, dSrcs, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(dFarS, 0, n_srcs * 8, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(dReachS, 0, n_srcs * 4, st);
     p.srcs = dSrcs;
@@ -714,10 +866,12 @@ static int closeness_impl(blest_handle_t h, const uint32_t* srcs, uint64_t n_src
     p.farT = h->dFarT;
     p.reachT = h->dReachT;
   }
-  if (e == cudaSuccess && cc && !ccDev) e = talloc((void**)&dCc, n_srcs * 8);
-  if (e == cudaSuccess && farOut && !farDev) e = talloc((void**)&dFarO, n_srcs * 8);
-  if (e == cudaSuccess && reachOut && !reachDev) e = talloc((void**)&dReachO, n_srcs * 4);
+  if (e == cudaSuccess && cc && !ccDev) e = tmp.alloc((void**)&dCc, n_srcs * 8);
+  if (e == cudaSuccess && farOut && !farDev) e = tmp.alloc((void**)&dFarO, n_srcs * 8);
+  if (e == cudaSuccess && reachOut && !reachDev) e = tmp.alloc((void**)&dReachO, n_srcs * 4);
+  h->lastCtrl = h->dCtrl;
   if (e == cudaSuccess) e = cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->dMsStats, 0, 8 * sizeof(unsigned long long), st);
   if (e == cudaSuccess) e = launch_msbfs(p, h->gridMs, st);
   if (e == cudaSuccess)
     e = launch_closeness_finalize(h->n, h->rho, h->hasPerm ? h->dPerm : nullptr, p.farT, p.reachT, p.farS, p.reachS, n_srcs,
@@ -727,14 +881,58 @@ static int closeness_impl(blest_handle_t h, const uint32_t* srcs, uint64_t n_src
   if (e == cudaSuccess && cc && !ccDev) e = cudaMemcpyAsync(cc, dCc, n_srcs * 8, cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess && farOut && !farDev) e = cudaMemcpyAsync(farOut, dFarO, n_srcs * 8, cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess && reachOut && !reachDev) e = cudaMemcpyAsync(reachOut, dReachO, n_srcs * 4, cudaMemcpyDeviceToHost, st);
-  const bool needSync = !tmp.empty();
-  if (e == cudaSuccess && needSync) e = cudaStreamSynchronize(st);
-  cleanup();
-  if (e != cudaSuccess) {
-    g_lastCuda = (int)e;
-    cudaGetLastError();
-    return e == cudaErrorMemoryAllocation ? BLEST_ENOMEM : BLEST_ECUDA;
-  }
+  tmp.release();  // stream-ordered
+  if (e != cudaSuccess) return ms_fail(e);
+  return BLEST_OK;
+}
+
+int blest_farness_partial(blest_handle_t h, uint32_t first, uint32_t count, uint64_t* far_sum, uint32_t* reach_sum,
+                          void* cuda_stream) {
+  if (!h || !far_sum || !reach_sum || count == 0) return BLEST_EINVAL;
+  if (h->hostOnly) return BLEST_EUNSUPPORTED;
+  if ((uint64_t)first + count > h->n) return BLEST_EINVAL;
+  if (!is_device_ptr(far_sum) || !is_device_ptr(reach_sum)) return BLEST_EINVAL;
+  if (int rc = pending_status(h)) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = ensure_ms_workspace(h);
+  if (rc) return rc;
+  MsParams p{};
+  fill_ms_params(h, p);
+  p.srcBase = first;
+  p.nsrcs = count;
+  p.farT = h->dFarT;
+  p.reachT = h->dReachT;
+  h->lastCtrl = h->dCtrl;
+  cudaError_t e = cudaMemsetAsync(h->dFarT, 0, (size_t)h->rho * 8u * 8u, st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->dReachT, 0, (size_t)h->rho * 8u * 4u, st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->dMsStats, 0, 8 * sizeof(unsigned long long), st);
+  if (e == cudaSuccess) e = launch_msbfs(p, h->gridMs, st);
+  // target-side sums in ORIGINAL vertex ids (the finalize kernel maps id -> getVI(perm[id]))
+  if (e == cudaSuccess)
+    e = launch_closeness_finalize(h->n, h->rho, h->hasPerm ? h->dPerm : nullptr, p.farT, p.reachT, nullptr, nullptr, h->n,
+                                  nullptr, (unsigned long long*)far_sum, reach_sum, st);
+  if (e != cudaSuccess) return ms_fail(e);
+  return BLEST_OK;
+}
+
+int blest_closeness_from_sums(const uint64_t* far_sum, const uint32_t* reach_sum, uint64_t n, double* out, void* cuda_stream) {
+  if (!far_sum || !reach_sum || !out || n == 0) return BLEST_EINVAL;
+  if (!is_device_ptr(far_sum) || !is_device_ptr(reach_sum) || !is_device_ptr(out)) return BLEST_EINVAL;
+  cudaError_t e = launch_closeness_finalize((uint32_t)std::min<uint64_t>(n, 0xFFFFFFFFull), 0, nullptr, nullptr, nullptr,
+                                            (const unsigned long long*)far_sum, reach_sum, n, out, nullptr, nullptr,
+                                            (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return ms_fail(e);
+  return BLEST_OK;
+}
+
+int blest_get_ms_stats(blest_handle_t h, uint64_t* out8) {
+  if (!h || !out8) return BLEST_EINVAL;
+  if (h->hostOnly) return BLEST_EUNSUPPORTED;
+  for (int k = 0; k < 8; ++k) out8[k] = 0;
+  if (!h->dMsStats) return BLEST_OK;
+  CK(cudaDeviceSynchronize());
+  CK(cudaMemcpy(out8, h->dMsStats, 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost));
   return BLEST_OK;
 }
 
@@ -827,6 +1025,39 @@ int blest_mma_microbench(int kind, uint32_t iters, double* tera_macs_per_s, doub
   CK(e);
   *tera_macs_per_s = macs / (best * 1e-3) / 1e12;
   if (milliseconds) *milliseconds = best;
+  return BLEST_OK;
+}
+
+int blest_l2_microbench(uint64_t bytes, uint32_t iters, double* gb_per_s) {
+  if (!gb_per_s || iters == 0 || bytes < 4096) return BLEST_EINVAL;
+  int dev = 0, sms = 0;
+  CK(cudaGetDevice(&dev));
+  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const uint64_t n16 = bytes / 32;  // half the footprint is read, half written
+  uint4 *a = nullptr, *b = nullptr;
+  CK(cudaMalloc((void**)&a, n16 * 16));
+  cudaError_t e = cudaMalloc((void**)&b, n16 * 16);
+  if (e == cudaSuccess) e = cudaMemset(a, 1, n16 * 16);
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  if (e == cudaSuccess) e = run_l2_copy(a, b, n16, 2, sms);  // warm-up: both buffers become L2-resident
+  float best = 1e30f;
+  for (int rep = 0; rep < 5 && e == cudaSuccess; ++rep) {
+    cudaEventRecord(e0);
+    e = run_l2_copy(a, b, n16, iters, sms);
+    cudaEventRecord(e1);
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    best = std::min(best, ms);
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(a);
+  if (b) cudaFree(b);
+  CK(e);
+  *gb_per_s = (double)n16 * 32.0 * iters / (best * 1e-3) / 1e9;
   return BLEST_OK;
 }
 

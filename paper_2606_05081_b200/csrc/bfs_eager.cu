@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_eager_kernel(const __gri
     if (nent <= p.qcap) {
       for (uint32_t i = lane; i < nent; i += 32) write_entry(p.Q[1], 0, 0, a, nq, s0, i);
       if (lane == 0) ctrl->tail = nent;
-    } else if (lane == 0) atomicOr(&ctrl->error, 1u);
+    } else if (lane == 0) report_overflow(ctrl, p.hostStatus);
   }
   // The queue tail is ONE monotone counter: the entries of level l+1 take positions [tEnd_l, tEnd_{l+1}) and live in
   // Q[(l+1) & 1] at (position - tEnd_l).  The barrier hands every CTA the tail, so no queue length is read or reset.
@@ -67,7 +67,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_eager_kernel(const __gri
 
   uint32_t level = 1;
   for (;; ++level) {
-    const uint32_t qcount = tEnd - tStart;
+    const uint32_t qcount = min(tEnd - tStart, p.qcap);  // (after an overflow the tail counts entries that were dropped)
     if (qcount == 0) break;
     const uint2* Qc = p.Q[level & 1u];
     uint2* Qn = p.Q[(level + 1) & 1u];
@@ -123,7 +123,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_eager_kernel(const __gri
       {  // capacity of the next level's queue (the tail itself never wraps: every VSS is enqueued <= 8 times per call)
         const uint32_t tot = __reduce_add_sync(0xffffffffu, cnt), first = __shfl_sync(0xffffffffu, pos, 0);
         ok = tot == 0u || (uint64_t)first + tot <= p.qcap;
-        if (!ok && lane == 0) atomicOr(&ctrl->error, 1u);
+        if (!ok && lane == 0) report_overflow(ctrl, p.hostStatus);
       }
       if (ok)
         for (uint32_t k = 0; k < nseg; ++k) emit_segment(Qn, pos, 0, segA[k], segN[k], segS[k], bigList, bigCnt);

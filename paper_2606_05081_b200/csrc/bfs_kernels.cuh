@@ -48,6 +48,7 @@ struct BfsParams {
   int gather;              // lazy kernel: final pass out[v] = lvl[perm[v]]
   int32_t* L;      // levels in internal ids (== out when there is no reordering)
   Ctrl* ctrl;
+  unsigned int* hostStatus;  // host-mapped latch of the handle (overflow report), may be nullptr
   blest_level_trace_t* trace;
   uint32_t traceCap;
   uint32_t src;      // internal id
@@ -75,8 +76,12 @@ struct MsParams {
   uint8_t* dirty;  // Ns
   uint2* Q[2];
   Ctrl* ctrl;
-  const uint32_t* srcs;  // device, original ids; nullptr = identity (source i = vertex i)
+  unsigned int* hostStatus;  // host-mapped latch of the handle (overflow report), may be nullptr
+  const uint32_t* srcs;  // device, original ids; nullptr = identity (source i = vertex srcBase + i)
+  uint64_t srcBase;      // first vertex of the source range when srcs == nullptr (multi-GPU partition)
   uint64_t nsrcs;
+  unsigned long long* stats;  // optional [8]: totals of the launch for the roofline (queue entries, quads, slices probed,
+                              // fresh row updates, dirty slice sets swept, levels, batches)
   // outputs (any may be nullptr)
   int32_t* levels;              // [nsrcs][n] original ids
   unsigned long long* farT;     // target-side accumulation, indexed by getVI(internal id) (Eq. 7)

@@ -300,7 +300,7 @@ __device__ __forceinline__ void emit_chunks(const BfsParams& p, Ctrl* ctrl, uint
   }
   pos = __shfl_sync(FULL, pos, 0);
   if ((uint64_t)pos + nent > p.chunkCap) {
-    if (lane == 0) atomicOr(&ctrl->error, 1u);
+    if (lane == 0) report_overflow(ctrl, p.hostStatus);
     return;
   }
   for (uint32_t i = lane; i < nent; i += 32) p.chunks[pos + i] = make_uint4(start + i * per, min(per, count - i * per), alpha, type);
@@ -874,8 +874,12 @@ template <int CONTR>
 __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid_constant__ BfsParams p) {
   extern __shared__ __align__(16) unsigned char lazy_smem[];
   LazyShared& sh = *reinterpret_cast<LazyShared*>(lazy_smem);
-  unsigned int epoch = 0;
   Ctrl* ctrl = p.ctrl;
+  // The control block is never memset between calls: the barrier counter is monotone over the launches on this
+  // handle (stream-ordered), `epochBase` is where the previous launch left it, and the leader resets the per-call
+  // fields below.  Only thread 0 of a CTA evaluates the barrier target, so only it needs the true epoch.
+  unsigned int epoch = 0;
+  if (threadIdx.x == 0) epoch = ld_volatile(&ctrl->epochBase);
   const uint64_t gtid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (uint64_t)gridDim.x * blockDim.x;
   const bool leader = (blockIdx.x == 0 && threadIdx.x == 0);
   if (threadIdx.x < 6) sh.acc[threadIdx.x] = 0;
@@ -907,6 +911,13 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
   const uint32_t srcRow = __ldg(&p.rowptr[p.src]);
   const uint32_t srcDeg = __ldg(&p.rowptr[p.src + 1]) - srcRow;
   if (leader) {
+    ctrl->error = 0;
+    ctrl->nlevels = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      ctrl->qc[k] = 0; ctrl->qbytes[k] = 0; ctrl->unvisited[k] = 0; ctrl->newcount[k] = 0;
+      ctrl->mf[k] = 0; ctrl->buScanned[k] = 0; ctrl->wlc[k] = 0; ctrl->nBig[k] = 0;
+    }
     // level 0: the source itself (frontier = {src})
     p.WL[0][0] = srcWord;
     ctrl->wlc[0] = 1;
@@ -958,14 +969,16 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     }
     unsigned long long tStage1 = 0;
     if (level == 1 && !bottomUp && p.switching == 0) {
-      // Level 1 needs no probe, no filter and no sweep: the neighbours of the source are distinct and all unvisited, so
-      // each edge of the source finalises its target on the spot (one phase, one barrier instead of two and a sweep).
+      // Level 1 needs no probe, no filter and no sweep: the neighbours of the source other than itself are all unvisited,
+      // so each edge of the source finalises its target on the spot (one phase, one barrier instead of two and a sweep);
+      // a duplicated CSR entry is caught by the returning atomic on F_next.
       Counters c;
       const uint32_t lane = threadIdx.x & 31;
       const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
       for (uint32_t base = gwarp * 32u; base < srcDeg; base += nwarps * 32u) {
-        const bool active = base + lane < srcDeg;
+        bool active = base + lane < srcDeg;
         const uint32_t v = active ? __ldcs(p.colidx + srcRow + base + lane) : 0u;
+        active = active && v != p.src;  // a self-loop (src, src) discovers nothing: the source is the only visited vertex
         const uint32_t bit = 1u << (v & 31u);
         uint32_t old = FULL;
         if (active) old = atomicOr(&Fn[v >> 5], bit);
@@ -1030,7 +1043,10 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       p.trace[level - 1] = r;
     }
   }
-  if (leader) ctrl->nlevels = level - 1;
+  if (leader) {
+    ctrl->nlevels = level - 1;
+    ctrl->epochBase = epoch;  // every CTA has executed the same barriers: the next launch continues from here
+  }
 
   // A10 as a separate pass (p.gather): the levels were written in internal ids (coalesced, no iperm read) and go to
   // original ids here.  Used when levels_out is too big to be held in L2 by the persisting window: scattered 4-byte

@@ -32,7 +32,17 @@ struct Ctrl {
   unsigned long long tInit;         // lazy kernel: ns from kernel start to the end of the per-call init
   unsigned int wlc[4];              // lazy kernel: frontier word-list lengths (rotating, level mod 3)
   unsigned int nBig[4];             // lazy kernel: deferred big segments of the level (rotating)
+  unsigned int epochBase;           // lazy kernel: grid barriers executed by earlier launches on this control block.  That
+                                    // kernel's block is zeroed once at build; every launch resets the per-call fields
+                                    // itself and leaves `bar` = epochBase * gridDim (mod 2^32), so no memset precedes a call
 };
+
+// Work-queue overflow: flagged in the control block of the call (blest_get_trace) and latched in the handle's
+// host-mapped status word (blest_last_status; include/blest.h "Asynchrony").
+__device__ __forceinline__ void report_overflow(Ctrl* ctrl, unsigned int* hostStatus) {
+  atomicOr(&ctrl->error, 1u);
+  if (hostStatus) *(volatile unsigned int*)hostStatus = 1u;
+}
 
 __device__ __forceinline__ unsigned long long globaltimer() {
   unsigned long long t;
@@ -51,7 +61,7 @@ __device__ __forceinline__ void grid_barrier(unsigned int* bar, unsigned int& ep
     unsigned int v;
     do {
       asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
-    } while (v < target);
+    } while ((int)(v - target) < 0);  // wrap-safe: the counter is monotone over billions of barriers (closeness runs)
   }
   __syncthreads();
 }
@@ -67,15 +77,13 @@ __device__ __forceinline__ unsigned int grid_barrier_tail(unsigned int* bar, uns
     unsigned long long v;
     do {
       asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(bar) : "memory");
-    } while ((unsigned int)v < target);
+    } while ((int)((unsigned int)v - target) < 0);  // wrap-safe, as above
     *slot = (unsigned int)(v >> 32);
   }
   __syncthreads();
   return *slot;
 }
 
-template <class T>
-__device__ __forceinline__ T ld_cg(const T* p) { return __ldcg(p); }
 __device__ __forceinline__ unsigned int ld_volatile(const unsigned int* p) { return *(const volatile unsigned int*)p; }
 __device__ __forceinline__ unsigned long long ld_volatile(const unsigned long long* p) {
   return *(const volatile unsigned long long*)p;

@@ -21,7 +21,7 @@ int check_csr(const HostCsr& g, bool validate_symmetry) {
 #pragma omp parallel for schedule(dynamic, 4096) reduction(| : bad)
   for (int64_t i = 0; i < (int64_t)n; ++i) {
     uint32_t b = g.rowptr[i], e = g.rowptr[i + 1];
-    if (e < b) { bad |= 2; continue; }
+    if (e < b || e > g.nnz) { bad |= 2; continue; }  // malformed rowptr: never walk colidx past nnz
     for (uint32_t p = b; p < e; ++p) {
       if (g.colidx[p] >= n) bad |= 4;
       if (p > b && g.colidx[p] < g.colidx[p - 1]) bad |= 1;

@@ -7,7 +7,6 @@ namespace blest {
 
 constexpr uint32_t SIGMA = 8;          // slice width sigma
 constexpr uint32_t THETA = 4;          // slices per lane, theta = 32 / sigma
-constexpr uint32_t TAU = 128;          // slices per VSS, tau = 32 * theta
 constexpr uint32_t QUADS_PER_VSS = 32; // one quad (4 slices) per lane
 
 struct HostCsr {

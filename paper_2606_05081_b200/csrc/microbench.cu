@@ -63,7 +63,27 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) barrier_bench_kernel(unsigne
   if (blockIdx.x == 0 && threadIdx.x == 0) *nsOut = t1 - t0;
 }
 
+// L2 bandwidth: `iters` passes of a 16-byte-per-thread copy over buffers small enough to stay L2-resident (read + write
+// bytes are counted); the launch configuration of the persistent kernels (one 1024-thread CTA per SM).
+__global__ void __launch_bounds__(BLOCK_THREADS, 1) l2_copy_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst,
+                                                                   uint64_t n16, uint32_t iters) {
+  const uint64_t tid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (uint64_t)gridDim.x * blockDim.x;
+  for (uint32_t it = 0; it < iters; ++it) {
+    uint64_t i = tid;
+    for (; i + 3 * nth < n16; i += 4 * nth) {  // four independent 16-byte loads in flight per thread
+      const uint4 a = __ldcg(src + i), b = __ldcg(src + i + nth), c = __ldcg(src + i + 2 * nth), d = __ldcg(src + i + 3 * nth);
+      dst[i] = a; dst[i + nth] = b; dst[i + 2 * nth] = c; dst[i + 3 * nth] = d;
+    }
+    for (; i < n16; i += nth) dst[i] = __ldcg(src + i);
+  }
+}
+
 }  // namespace
+
+cudaError_t run_l2_copy(const uint4* src, uint4* dst, uint64_t n16, uint32_t iters, int blocks) {
+  l2_copy_kernel<<<blocks, BLOCK_THREADS>>>(src, dst, n16, iters);
+  return cudaGetLastError();
+}
 
 cudaError_t run_contraction_selftest(int contraction, unsigned long long* dMismatch) {
   switch (contraction) {

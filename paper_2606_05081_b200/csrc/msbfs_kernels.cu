@@ -23,6 +23,8 @@ struct MsShared {
   unsigned int tailSlot;  // broadcast slot of grid_barrier_tail
   uint32_t perSource[256];
   uint32_t fset[WARPS_PER_BLOCK][8 * 8];  // per warp: the kappa-bit frontier words of the current set's 8 columns
+  unsigned long long cnt[WARPS_PER_BLOCK][5];  // per warp (lane 0): queue entries, quads, slices probed, fresh row
+                                               // updates, dirty slice sets swept -- totals for the roofline (p.stats)
 };
 
 // One kappa-bit word (KW 32-bit words, naturally aligned) moved with a single vector access.
@@ -90,6 +92,7 @@ __device__ __forceinline__ void ms_stage1(const MsParams& p, MsShared& sh, const
     }
     __syncwarp();
     const uint32_t ru[4] = {rows.x, rows.y, rows.z, rows.w};
+    uint32_t nProbe = 0, nFresh = 0;
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
       const uint32_t mb = (m >> (8 * c)) & 0xFFu;
@@ -110,14 +113,23 @@ __device__ __forceinline__ void ms_stage1(const MsParams& p, MsShared& sh, const
         if (any) {  // one probe and one RED per row, each a single kappa-bit access
           uint32_t vn[KW], fresh[KW];
           load_words<KW>(p.Vn, idx, vn);
+          ++nProbe;
           any = 0;
 #pragma unroll
           for (int w = 0; w < KW; ++w) { fresh[w] = M[w] & ~vn[w]; any |= fresh[w]; }
           if (any) {
             red_or_words<KW>(p.Vn, idx, fresh);
             p.dirty[u >> 3] = 1;  // PAPER.md:583 dirtySets
+            ++nFresh;
           }
         }
+      }
+    }
+    if (p.stats) {
+      const uint32_t tp = __reduce_add_sync(0xffffffffu, nProbe), tf = __reduce_add_sync(0xffffffffu, nFresh);
+      if (lane == 0) {
+        unsigned long long* cnt = sh.cnt[threadIdx.x >> 5];
+        cnt[0] += 1; cnt[1] += nq; cnt[2] += tp; cnt[3] += tf;
       }
     }
   }
@@ -134,7 +146,12 @@ __device__ __forceinline__ void ms_stage2(const MsParams& p, MsShared& sh, uint3
   for (uint64_t sb = (uint64_t)gwarp * 32; sb < p.Ns; sb += (uint64_t)nwarps * 32) {
     const uint32_t s = (uint32_t)sb + lane;  // consecutive threads -> consecutive slice sets
     uint32_t cnt = 0, a = 0, nq = 0;
-    if (s < p.Ns && p.dirty[s]) {  // skip slice sets nobody marked
+    const bool isDirty = s < p.Ns && p.dirty[s];
+    if (p.stats) {
+      const uint32_t nd = __popc(__ballot_sync(0xffffffffu, isDirty));
+      if (lane == 0) sh.cnt[warp][4] += nd;
+    }
+    if (isDirty) {  // skip slice sets nobody marked
       p.dirty[s] = 0;
       uint32_t A = 0;
       constexpr uint32_t R = KW <= 2 ? 8u : (KW == 4 ? 4u : 2u);  // rows whose words are in flight together
@@ -191,7 +208,7 @@ __device__ __forceinline__ void ms_stage2(const MsParams& p, MsShared& sh, uint3
     {
       const uint32_t tot = __reduce_add_sync(0xffffffffu, cnt), first = __shfl_sync(0xffffffffu, pos, 0);
       ok = tot == 0u || (uint64_t)first + tot <= p.qcap;
-      if (!ok && lane == 0) atomicOr(&p.ctrl->error, 1u);
+      if (!ok && lane == 0) report_overflow(p.ctrl, p.hostStatus);
     }
     if (cnt && ok) emit_segment(Qn, pos, 0, a, nq, s, bigList, bigCnt);
     flush_big_segments(Qn, bigList, bigCnt, lane);
@@ -219,8 +236,10 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_co
   if (threadIdx.x < WARPS_PER_BLOCK) sh.bigCnt[threadIdx.x] = 0;
   if (threadIdx.x < 256) sh.perSource[threadIdx.x] = 0;
   if (threadIdx.x == 0) sh.acc = 0;
+  if (threadIdx.x < WARPS_PER_BLOCK * 5) sh.cnt[threadIdx.x / 5][threadIdx.x % 5] = 0;
   __syncthreads();
   const uint64_t stateWords = (uint64_t)p.rho * 8u * KW;
+  unsigned long long nLevels = 0, nBatches = 0;
 
   uint32_t tStart = 0, tEnd = 0;  // queue tail before / after the sweep that filled the current level's queue
   for (uint64_t b0 = 0; b0 < p.nsrcs; b0 += KAPPA) {
@@ -235,7 +254,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_co
     grid_barrier(&ctrl->bar, epoch);
     if (gtid < nb) {
       const uint32_t c = (uint32_t)gtid;
-      const uint32_t so = p.srcs ? p.srcs[b0 + c] : (uint32_t)(b0 + c);
+      const uint32_t so = p.srcs ? p.srcs[b0 + c] : (uint32_t)(p.srcBase + b0 + c);
       const uint32_t si = p.perm ? __ldg(&p.perm[so]) : so;
       const uint64_t idx = (uint64_t)(si & 7u) * p.rho + (si >> 3);
       atomicOr(&p.Vn[idx * KW + (c >> 5)], 1u << (c & 31u));
@@ -253,8 +272,9 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_co
       const uint32_t par = level & 1u;
       // a level whose sweep enqueued nothing discovered nothing (every discovered vertex has a neighbour, so its slice
       // set has slices): the queue length the barrier returned is the termination test
-      const uint32_t qcount = tEnd - tStart;
+      const uint32_t qcount = min(tEnd - tStart, p.qcap);  // (after an overflow the tail counts dropped entries)
       if (qcount == 0) break;
+      ++nLevels;
       ms_stage1<KW>(p, sh, p.Q[par], qcount);
       grid_barrier(&ctrl->bar, epoch);
       ms_stage2<KW>(p, sh, level, b0, nb, p.Q[par ^ 1u], tEnd);
@@ -262,6 +282,17 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_co
       tStart = tEnd;
       tEnd = t;
     }
+    ++nBatches;
+  }
+  if (p.stats) {
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) {
+      const unsigned long long* cnt = sh.cnt[threadIdx.x >> 5];
+#pragma unroll
+      for (int k = 0; k < 5; ++k)
+        if (cnt[k]) atomicAdd(&p.stats[k], cnt[k]);
+    }
+    if (gtid == 0) { p.stats[5] = nLevels; p.stats[6] = nBatches; }
   }
 }
 

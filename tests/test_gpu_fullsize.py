@@ -10,11 +10,21 @@ import oracle
 
 pytestmark = pytest.mark.gpu
 
+
+_CACHE = {}
+
+
+def config_graph(name):
+    """One generated CSR per config for the whole module (config 4 takes 20 s to generate; all four are < 6 GB)."""
+    if name not in _CACHE:
+        _CACHE[name] = gg.make_config(name)
+    return _CACHE[name]
+
 # reorder as in bench.py (REORDER_FOR); number of sources compared element-wise / by (far, reach)
 FULL = {
     "c2_grid4096": dict(reorder="none", n_levels=2, n_far=2),
     "c3_gnm25": dict(reorder="none", n_levels=2, n_far=4),
-    "c4_rmat24": dict(reorder="degree", n_levels=3, n_far=8),
+    "c4_rmat24": dict(reorder="degree", n_levels=3, n_far=0),   # all 64 by (far, reach) in the test below
 }
 
 
@@ -33,7 +43,7 @@ def env():
 def test_full_size_levels_and_farness(env, name):
     torch, blest = env
     cfg = FULL[name]
-    n, rp, ci = gg.make_config(name)
+    n, rp, ci = config_graph(name)
     srcs = gg.config_sources(name, rp)
     out = torch.empty(n, dtype=torch.int32, device="cuda")
     with blest.Graph(n, rp, ci, reorder=cfg["reorder"]) as g:
@@ -53,12 +63,59 @@ def test_full_size_levels_and_farness(env, name):
                 far, reach = oracle.farness(lv)  # plain sum / count of the GPU's level array
                 assert (far, reach) == (int(fw), int(rw)), f"{name} src {int(s)}"
                 assert lv[int(s)] == 0 and lv.min() >= -1
+        assert g.last_status() == 0
+
+
+def test_full_size_c4_all_sources_and_odd_components(env):
+    """Config 4 in bench.py's launch configuration: farness / reach of ALL 64 timed sources against the oracle, plus
+    sources the seeded draw does not contain: one outside the hub's component (RMAT leaves a few two- and three-vertex
+    components) and, with the component pruning switched off, the same sources again."""
+    torch, blest = env
+    n, rp, ci = config_graph("c4_rmat24")
+    srcs = gg.config_sources("c4_rmat24", rp)
+    deg = gg.degrees(rp)
+    giant = oracle.bfs(n, rp, ci, int(np.argmax(deg))) >= 0
+    small = np.flatnonzero(~giant & (deg > 0))                       # vertices of the small components
+    assert small.size > 0
+    odd = np.array([small[0], small[-1], np.flatnonzero(deg == 0)[0]], dtype=np.uint32)
+    all_srcs = np.concatenate([srcs, odd]).astype(np.uint32)
+    far_w, reach_w, _, _ = oracle.closeness(n, rp, ci, all_srcs)
+    out = torch.empty(n, dtype=torch.int32, device="cuda")
+    for prune in (True, False):
+        with blest.Graph(n, rp, ci, reorder="degree", prune_components=prune) as g:
+            assert (g.info().component_seconds > 0) == prune
+            todo = all_srcs if prune else np.concatenate([srcs[:4], odd])
+            for s in todo:
+                g.bfs(int(s), out)
+                lv = out.cpu().numpy()
+                i = int(np.flatnonzero(all_srcs == s)[0])
+                assert oracle.farness(lv) == (int(far_w[i]), int(reach_w[i])), f"src {int(s)} prune {prune}"
+                assert lv[int(s)] == 0 and lv.min() >= -1
+            for s in odd[:2]:                                          # element-wise on the small components
+                g.bfs(int(s), out)
+                assert np.array_equal(out.cpu().numpy(), oracle.bfs(n, rp, ci, int(s)))
+            assert g.last_status() == 0
+
+
+@pytest.mark.parametrize("contraction", ["mma_b1", "mma_u8"])
+def test_mma_contraction_forms_on_c4_shrunk(env, contraction):
+    """The tensor-core contraction forms inside a traversal of a graph with hub slice sets (config 4 at scale 20),
+    slice path forced on every level."""
+    torch, blest = env
+    n, rp, ci = gg.make_config("c4_rmat24", 4)
+    srcs = gg.config_sources("c4_rmat24", rp)[:3]
+    out = torch.empty(n, dtype=torch.int32, device="cuda")
+    with blest.Graph(n, rp, ci, reorder="degree", switching="off", contraction=contraction) as g:
+        for s in srcs:
+            g.bfs(int(s), out)
+            assert np.array_equal(out.cpu().numpy(), oracle.bfs(n, rp, ci, int(s))), (contraction, int(s))
+        assert g.last_status() == 0
 
 
 def test_full_size_c3_rcm(env):
     """Config 3 'with and without RCM reordering before BVSS build': the reordered run gives the same levels."""
     torch, blest = env
-    n, rp, ci = gg.make_config("c3_gnm25")
+    n, rp, ci = config_graph("c3_gnm25")
     s = int(gg.config_sources("c3_gnm25", rp)[0])
     out = torch.empty(n, dtype=torch.int32, device="cuda")
     with blest.Graph(n, rp, ci, reorder="rcm") as g:
@@ -66,15 +123,17 @@ def test_full_size_c3_rcm(env):
         assert np.array_equal(out.cpu().numpy(), oracle.bfs(n, rp, ci, s))
 
 
-def test_full_size_c5_closeness_sampled(env):
-    """Config 5: all 262 144 vertices are sources (kappa = 64 batches); farness / reach bit-exact and closeness equal to
-    the oracle's IEEE division on a seeded sample of 512 sources (incl. isolated vertices)."""
+@pytest.mark.parametrize("kappa", [64, 128, 256])
+def test_full_size_c5_closeness_sampled(env, kappa):
+    """Config 5: all 262 144 vertices are sources (kappa-wide batches); farness / reach bit-exact and closeness equal to
+    the oracle's IEEE division on a seeded sample of 512 sources (incl. isolated vertices), for every width the
+    sources-per-second figures are quoted at."""
     torch, blest = env
-    n, rp, ci = gg.make_config("c5_rmat18")
+    n, rp, ci = config_graph("c5_rmat18")
     rng = np.random.Generator(np.random.PCG64(5))
     sample = np.sort(rng.choice(n, size=512, replace=False)).astype(np.uint32)
     far_w, reach_w, cc_w, _ = oracle.closeness(n, rp, ci, sample)
-    with blest.Graph(n, rp, ci, kappa=64) as g:
+    with blest.Graph(n, rp, ci, kappa=kappa) as g:
         far = torch.zeros(n, dtype=torch.int64, device="cuda")
         reach = torch.zeros(n, dtype=torch.int32, device="cuda")
         g.farness(far, reach)
@@ -83,6 +142,12 @@ def test_full_size_c5_closeness_sampled(env):
         far_g = far.cpu().numpy().view(np.uint64)
         reach_g = reach.cpu().numpy().view(np.uint32)
         cc_g = cc.cpu().numpy()
+        assert g.last_status() == 0
+        if kappa == 64:  # a source subset at full size: per-source counts (reading R13)
+            sub = sample[:96]
+            f2, r2 = np.zeros(sub.size, dtype=np.uint64), np.zeros(sub.size, dtype=np.uint32)
+            g.farness(f2, r2, srcs=sub)
+            assert np.array_equal(f2, far_w[:96]) and np.array_equal(r2, reach_w[:96])
     assert np.array_equal(far_g[sample], far_w)
     assert np.array_equal(reach_g[sample], reach_w)
     assert np.allclose(cc_g[sample], cc_w, rtol=1e-12, atol=0.0)
@@ -90,8 +155,7 @@ def test_full_size_c5_closeness_sampled(env):
     # properties that hold for every source: reach >= 1; far = 0 iff reach = 1; closeness in [0, 1]
     assert reach_g.min() >= 1 and np.array_equal(far_g == 0, reach_g == 1)
     assert cc_g.min() >= 0.0 and cc_g.max() <= 1.0
-    # sum over sources of far = sum over targets of far (undirected graph): both are the same all-pairs sum, and the
-    # component sizes agree: every vertex of a component reports the same reach
+    # the component sizes agree: every vertex of a component reports the same reach
     lv = oracle.bfs(n, rp, ci, int(sample[np.argmax(reach_w)]))
     comp = lv >= 0
     assert np.all(reach_g[comp] == reach_g[comp][0])
