@@ -350,8 +350,9 @@ def forced_slice_extra(g, torch, srcs, edges, n, reordered, sweep_words, peak, s
     ref = []
     for s in srcs[:k]:
         g.bfs(int(s), out, stream=stream)
+        with torch.cuda.stream(stream):  # (the copy must be ordered before the next traversal overwrites `out`)
+            ref.append(out.clone())
         stream.synchronize()
-        ref.append(out.clone())
     g.configure(switching="off")
     walg, same = 0, True
     for i, s in enumerate(srcs[:k]):

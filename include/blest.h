@@ -65,7 +65,8 @@ typedef struct {
  * can be changed later with blest_configure (so that every path can be forced on one handle: the
  * policy-independence tests and the ablation axes of PAPER.md Tables 4/6). */
 typedef struct {
-  int reorder;     /* 0 none | 1 RCM | 2 degree-descending (BASELINE.json config 4) */
+  int reorder;     /* 0 none | 1 RCM | 2 degree-descending (BASELINE.json config 4) |
+                      3 JaccardWithWindows (Alg. 1, W = 2^16) applied to the degree order */
   int builder;     /* 0 host (OpenMP over slice sets).  No other builder exists: any other value is BLEST_EINVAL */
   int validate;    /* 0 | 1: O(nnz log d) symmetry + range check */
   int kernel;      /* 0 auto by U_div | 1 eager (Alg. 2) | 2 lazy two-stage (Alg. 3) */
@@ -210,6 +211,12 @@ int blest_contraction_selftest(int contraction, uint64_t *n_mismatch);
  * reports tera-ops/s (one op = one multiply-accumulate on one bit (b1) or one byte (u8)), 2 ops per MAC not applied.
  * kind: 2 = mma.sync m8n8k128 b1 and.popc | 3 = mma.sync m16n8k32 u8. */
 int blest_mma_microbench(int kind, uint32_t iters, double *tera_macs_per_s, double *milliseconds);
+
+/* tcgen05.mma kind::i8 peak (the Blackwell tensor-core form north_star (b) names; operands in shared memory,
+ * accumulator in TMEM): `iters` MMAs of shape M = 128, N = n (16..256, multiple of 16), K = 32 per SM, issued by one
+ * thread per CTA; tera byte-MACs per second.  The accumulator is read back with tcgen05.ld and checked against
+ * 32 * iters for all-ones operands: *n_wrong = accumulator elements that differ (0 = the path works). */
+int blest_tcgen05_microbench(uint32_t iters, uint32_t n, double *tera_macs_per_s, uint64_t *n_wrong);
 
 /* L2 bandwidth microbenchmark (roofline denominator of the L2-resident multi-source path): a 16-byte-per-thread copy
  * between two buffers of bytes/2 each, `iters` passes, in the persistent launch configuration; read + write GB/s. */

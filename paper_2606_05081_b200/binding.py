@@ -22,7 +22,7 @@ _lib = None
 OK, EINVAL, ERANGE, EUNSORTED, ENOTSYM, ENOMEM, ECUDA, EUNSUPPORTED, EOVERFLOW = 0, -1, -2, -3, -4, -5, -6, -7, -8
 
 # option values
-REORDER = {"none": 0, "rcm": 1, "degree": 2}
+REORDER = {"none": 0, "rcm": 1, "degree": 2, "jaccard": 3}
 KERNEL = {"auto": 0, "eager": 1, "lazy": 2}
 SWITCHING = {"auto": 0, "off": 1, "bottom_up": 2, "top_down": 3, "slice": 4, "scripted": 5}
 CONTRACTION = {"auto": 0, "alu": 1, "mma_b1": 2, "mma_u8": 3}
@@ -71,7 +71,7 @@ TRACE_DTYPE = np.dtype([("level", "<u4"), ("mode", "<u4"), ("q_entries", "<u4"),
 
 EXPORTS = ["blest_build", "blest_preprocess_host", "blest_configure", "blest_get_call_stats", "blest_bfs", "blest_msbfs", "blest_closeness", "blest_farness",
            "blest_get_info", "blest_last_status", "blest_farness_partial", "blest_closeness_from_sums", "blest_get_ms_stats",
-           "blest_l2_microbench", "blest_get_trace", "blest_get_array", "blest_get_vi", "blest_contraction_selftest",
+           "blest_l2_microbench", "blest_tcgen05_microbench", "blest_get_trace", "blest_get_array", "blest_get_vi", "blest_contraction_selftest",
            "blest_mma_microbench", "blest_barrier_microbench", "blest_destroy", "blest_strerror",
            "blest_last_cuda_error"]
 
@@ -100,6 +100,7 @@ def load(build_if_missing: bool = True):
     L.blest_closeness_from_sums.argtypes = [vp, vp, u64, vp, vp]
     L.blest_get_ms_stats.argtypes = [vp, ctypes.POINTER(u64)]
     L.blest_l2_microbench.argtypes = [u64, u32, ctypes.POINTER(ctypes.c_double)]
+    L.blest_tcgen05_microbench.argtypes = [u32, u32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
     L.blest_get_trace.argtypes = [vp, vp, u32, ctypes.POINTER(u32)]
     L.blest_get_call_stats.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
     L.blest_get_array.argtypes = [vp, i32, vp, u64]
@@ -336,6 +337,13 @@ def l2_microbench(nbytes: int = 48 << 20, iters: int = 50) -> float:
     g = ctypes.c_double(0)
     _check(load().blest_l2_microbench(int(nbytes), int(iters), ctypes.byref(g)), "blest_l2_microbench")
     return g.value
+
+
+def tcgen05_microbench(iters: int = 2048, n: int = 256):
+    """(tera byte-MACs/s, wrong accumulator elements) of tcgen05.mma kind::i8, M = 128, N = n, K = 32."""
+    t, bad = ctypes.c_double(0), ctypes.c_uint64(0)
+    _check(load().blest_tcgen05_microbench(int(iters), int(n), ctypes.byref(t), ctypes.byref(bad)), "blest_tcgen05_microbench")
+    return t.value, int(bad.value)
 
 
 def barrier_microbench(iters: int = 2000) -> float:

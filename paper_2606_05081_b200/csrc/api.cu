@@ -16,6 +16,7 @@ cudaError_t run_contraction_selftest(int contraction, unsigned long long* dMisma
 cudaError_t run_mma_peak(int kind, uint32_t iters, int blocks, int* dSink, double* macsPerLaunch);
 cudaError_t run_barrier_bench(unsigned int* dBar, uint32_t iters, int blocks, unsigned long long* dNs);
 cudaError_t run_l2_copy(const uint4* src, uint4* dst, uint64_t n16, uint32_t iters, int blocks);
+cudaError_t run_tcgen05_peak(uint32_t iters, uint32_t n, int blocks, unsigned int* dBad, double* macsPerLaunch);
 }  // namespace blest
 
 using namespace blest;
@@ -119,7 +120,7 @@ static void normalise_options(blest_options_t& o) {
 }
 
 static int check_options(const blest_options_t& o) {
-  if (o.reorder < 0 || o.reorder > 2 || o.builder != 0) return BLEST_EINVAL;
+  if (o.reorder < 0 || o.reorder > 3 || o.builder != 0) return BLEST_EINVAL;
   if (o.persist_l2 < 0 || o.persist_l2 > 1 || o.prune_components < 0 || o.prune_components > 1) return BLEST_EINVAL;
   if (o.kernel < 0 || o.kernel > 2 || o.switching < 0 || o.switching > 5) return BLEST_EINVAL;
   if (o.contraction < 0 || o.contraction > 3) return BLEST_EINVAL;
@@ -394,7 +395,7 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
     }
     // scale-free-like test in the spirit of PAPER.md:199 (fn. 2: the top 1 % of the vertices hold a large share of the
     // degree); only meaningful after the degree sort, where the top vertices are the first ones
-    g->hubby = opt.reorder == 2 && g->nnz > 0 &&
+    g->hubby = (opt.reorder == 2 || opt.reorder == 3) && g->nnz > 0 &&
                (double)gcsr->rowptr[std::max<uint32_t>(g->n / 100u, 1u)] >= 0.20 * (double)g->nnz;
     g->realPtrs.swap(b.realPtrs);
     g->virtualToReal.swap(b.virtualToReal);
@@ -993,6 +994,41 @@ int blest_contraction_selftest(int contraction, uint64_t* n_mismatch) {
   cudaFree(d);
   CK(e);
   *n_mismatch = v;
+  return BLEST_OK;
+}
+
+int blest_tcgen05_microbench(uint32_t iters, uint32_t n, double* tera_macs_per_s, uint64_t* n_wrong) {
+  if (!tera_macs_per_s || !n_wrong || iters == 0 || n < 16 || n > 256 || (n & 15u)) return BLEST_EINVAL;
+  int dev = 0, sms = 0;
+  CK(cudaGetDevice(&dev));
+  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  unsigned int* dBad = nullptr;
+  CK(cudaMalloc((void**)&dBad, 4));
+  cudaError_t e = cudaMemset(dBad, 0, 4);
+  cudaEvent_t a, b;
+  cudaEventCreate(&a);
+  cudaEventCreate(&b);
+  double macs = 0;
+  if (e == cudaSuccess) e = run_tcgen05_peak(iters, n, sms, dBad, &macs);  // warm-up (and the correctness check)
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  float best = 1e30f;
+  for (int rep = 0; rep < 5 && e == cudaSuccess; ++rep) {
+    cudaEventRecord(a);
+    e = run_tcgen05_peak(iters, n, sms, dBad, &macs);
+    cudaEventRecord(b);
+    if (e == cudaSuccess) e = cudaEventSynchronize(b);
+    float ms = 0;
+    cudaEventElapsedTime(&ms, a, b);
+    best = std::min(best, ms);
+  }
+  unsigned int bad = 0;
+  if (e == cudaSuccess) e = cudaMemcpy(&bad, dBad, 4, cudaMemcpyDeviceToHost);
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  cudaFree(dBad);
+  CK(e);
+  *tera_macs_per_s = macs / (best * 1e-3) / 1e12;
+  *n_wrong = bad;
   return BLEST_OK;
 }
 

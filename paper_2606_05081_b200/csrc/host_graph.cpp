@@ -78,8 +78,104 @@ static void rcm_order(const HostCsr& g, std::vector<uint32_t>& order) {
   std::reverse(order.begin(), order.end());
 }
 
+// JaccardWithWindows (§4.1, Alg. 1, :116-184): the columns of every window of W consecutive ids are greedily
+// grouped into slice sets of sigma columns whose row neighbourhoods overlap (Eq. 3), so that the slices of a set carry
+// more than one bit (a denser mask = fewer slices = fewer BVSS bytes per edge).  `g` is symmetric, so nbrs_A = nbrs_A^T
+// = the sorted adjacency list, and nbrs(i) restricted to a window is a contiguous sub-range found by binary search.
+// slotOf[j] = new id of column j (the paper's pi^-1[j*] <- slot); windows run in parallel (Alg. 1 line 1).
+// Readings: "a highest-degree unassigned column" (lines 6, 13) breaks ties by the lowest id; a window's last slice set
+// may be short (n not a multiple of sigma); the listing is garbled in PAPER.md and follows the prose of :127-129.
+static void jaccard_with_windows(const HostCsr& g, uint32_t W, std::vector<uint32_t>& slotOf) {
+  const uint32_t n = g.n;
+  slotOf.assign(n, 0);
+  const int64_t nWin = ((int64_t)n + W - 1) / W;
+#pragma omp parallel
+  {
+    std::vector<uint64_t> inR(((size_t)n + 63) / 64, 0);  // membership of the current slice set's row set R
+    std::vector<uint32_t> rList, inter(W, 0), Q, byDeg(W);
+    std::vector<uint8_t> assigned(W, 0);
+#pragma omp for schedule(dynamic, 1)
+    for (int64_t w = 0; w < nWin; ++w) {
+      const uint32_t ws = (uint32_t)(w * W), we = (uint32_t)std::min<uint64_t>((uint64_t)ws + W, n), width = we - ws;
+      std::fill(assigned.begin(), assigned.begin() + width, 0);
+      for (uint32_t k = 0; k < width; ++k) byDeg[k] = ws + k;
+      std::stable_sort(byDeg.begin(), byDeg.begin() + width, [&](uint32_t a, uint32_t b) {
+        return (g.rowptr[a + 1] - g.rowptr[a]) > (g.rowptr[b + 1] - g.rowptr[b]);
+      });
+      uint32_t nextByDeg = 0;  // byDeg[nextByDeg..] holds every unassigned column at or after the best one
+      uint64_t sizeR = 0;
+      auto highest_unassigned = [&]() -> uint32_t {
+        while (assigned[byDeg[nextByDeg] - ws]) ++nextByDeg;
+        return byDeg[nextByDeg];
+      };
+      // R <- R u nbrs(j); every new row i bumps inter[] of the unassigned window columns it touches (Alg. 1 l.16-22 / l.9)
+      auto absorb = [&](uint32_t j) {
+        for (uint32_t e = g.rowptr[j]; e < g.rowptr[j + 1]; ++e) {
+          const uint32_t i = g.colidx[e];
+          if ((inR[i >> 6] >> (i & 63)) & 1ull) continue;
+          inR[i >> 6] |= 1ull << (i & 63);
+          rList.push_back(i);
+          ++sizeR;
+          const uint32_t* b = g.colidx.data() + g.rowptr[i];
+          const uint32_t* en = g.colidx.data() + g.rowptr[i + 1];
+          for (const uint32_t* q = std::lower_bound(b, en, ws); q < en && *q < we; ++q) {
+            const uint32_t k = *q - ws;
+            if (assigned[k]) continue;
+            if (inter[k]++ == 0) Q.push_back(*q);
+          }
+        }
+      };
+      for (uint32_t ss = ws; ss < we; ss += SIGMA) {
+        const uint32_t se = std::min(ss + SIGMA, we);
+        sizeR = 0;
+        uint32_t j = highest_unassigned();  // seed (line 6)
+        assigned[j - ws] = 1;
+        slotOf[j] = ss;
+        absorb(j);
+        for (uint32_t l = ss + 1; l < se; ++l) {
+          uint32_t best = 0xFFFFFFFFu;
+          double bestScore = -1.0;
+          size_t keep = 0;
+          for (size_t t = 0; t < Q.size(); ++t) {  // argmax over Q of inter / (|R| + deg - inter) (line 14)
+            const uint32_t c = Q[t];
+            if (assigned[c - ws]) continue;  // taken since it entered Q
+            Q[keep++] = c;
+            const double it = inter[c - ws], dg = g.rowptr[c + 1] - g.rowptr[c];
+            const double score = it / ((double)sizeR + dg - it);
+            if (score > bestScore || (score == bestScore && c < best)) { bestScore = score; best = c; }
+          }
+          Q.resize(keep);
+          j = best != 0xFFFFFFFFu ? best : highest_unassigned();  // Q empty: fallback (line 13)
+          assigned[j - ws] = 1;
+          slotOf[j] = l;
+          absorb(j);
+        }
+        for (uint32_t i : rList) inR[i >> 6] &= ~(1ull << (i & 63));
+        rList.clear();
+        for (uint32_t c : Q) inter[c - ws] = 0;
+        Q.clear();
+      }
+      std::fill(inter.begin(), inter.begin() + width, 0);
+    }
+  }
+}
+
 void make_permutation(const HostCsr& g, int kind, std::vector<uint32_t>& perm) {
   const uint32_t n = g.n;
+  if (kind == 3) {
+    // Degree order first, then JaccardWithWindows inside windows of the degree order: on a graph whose natural ids are a
+    // random relabelling (BASELINE.json's RMAT configs) a window of natural ids has no structure to exploit, while a
+    // window of the degree order holds columns of similar degree -- the hubs, whose neighbourhoods overlap most, first.
+    std::vector<uint32_t> p1, slotOf;
+    make_permutation(g, 2, p1);
+    HostCsr g1;
+    relabel_csr(g, p1, g1);
+    jaccard_with_windows(g1, JACCARD_WINDOW, slotOf);
+    perm.resize(n);
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < (int64_t)n; ++i) perm[i] = slotOf[p1[i]];
+    return;
+  }
   std::vector<uint32_t> order;  // order[new] = orig
   if (kind == 1) {
     rcm_order(g, order);

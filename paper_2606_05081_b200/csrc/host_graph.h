@@ -8,6 +8,7 @@ namespace blest {
 constexpr uint32_t SIGMA = 8;          // slice width sigma
 constexpr uint32_t THETA = 4;          // slices per lane, theta = 32 / sigma
 constexpr uint32_t QUADS_PER_VSS = 32; // one quad (4 slices) per lane
+constexpr uint32_t JACCARD_WINDOW = 1u << 16;  // W of JaccardWithWindows
 
 struct HostCsr {
   uint32_t n = 0;
@@ -31,7 +32,8 @@ struct HostBvss {
 
 // Status codes mirror include/blest.h.
 int check_csr(const HostCsr& g, bool validate_symmetry);
-// perm[orig] = new id.  kind: 1 RCM, 2 degree-descending (ties by id).
+// perm[orig] = new id.  kind: 1 RCM, 2 degree-descending (ties by id), 3 JaccardWithWindows (Alg. 1) on
+// top of the degree order.
 void make_permutation(const HostCsr& g, int kind, std::vector<uint32_t>& perm);
 void relabel_csr(const HostCsr& g, const std::vector<uint32_t>& perm, HostCsr& out);
 int build_bvss(const HostCsr& g, HostBvss& b);

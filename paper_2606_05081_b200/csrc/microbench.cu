@@ -78,7 +78,90 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) l2_copy_kernel(const uint4* 
   }
 }
 
+// ---- tcgen05.mma kind::i8 (5th-generation tensor cores, accumulator in TMEM): peak of the form north_star (b) names
+// as the alternative to mma.sync b1.  One CTA per SM; thread 0 issues `iters` MMAs of shape M = 128, N = n, K = 32
+// (int8 x int8 -> int32) on shared-memory operands that are all ones, commits them to an mbarrier, and the four warps
+// read the accumulator back with tcgen05.ld: every element must equal 32 * iters (independent of the operand layout,
+// so the check pins the instruction, the descriptors' reach and the TMEM read-back, not a particular swizzle).
+constexpr uint32_t TC_SMEM_BYTES = 48u << 10;  // operands + slack: any address the descriptors can generate holds ones
+
+__device__ __forceinline__ uint64_t umma_smem_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
+  // SM100 shared-memory matrix descriptor: start address >> 4 [0,14) | leading-dimension byte offset >> 4 [16,30) |
+  // stride-dimension byte offset >> 4 [32,46) | descriptor version 1 [46,48) | swizzle mode 0 = none [61,64)
+  return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo >> 4) << 16) | ((uint64_t)(sbo >> 4) << 32) | (1ull << 46);
+}
+
+__global__ void __launch_bounds__(128, 1) tcgen05_i8_peak_kernel(uint32_t iters, uint32_t n, unsigned int* bad) {
+  extern __shared__ __align__(1024) unsigned char tc_smem[];
+  __shared__ uint32_t tmemBase;
+  __shared__ __align__(8) uint64_t mbar;
+  for (uint32_t i = threadIdx.x; i < TC_SMEM_BYTES / 4; i += blockDim.x) reinterpret_cast<uint32_t*>(tc_smem)[i] = 0x01010101u;
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy stores -> visible to the tensor core's reads
+  const uint32_t warp = threadIdx.x >> 5;
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmemBase)), "r"(256u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  if (threadIdx.x == 0) {
+    mbar_init(&mbar, 1u);
+    mbar_init_fence();
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t taddr = tmemBase;
+  if (threadIdx.x == 0) {
+    // K-major, no swizzle: 8 x 16-byte core matrices, 128 B apart along K, 256 B apart along M / N
+    const uint64_t descA = umma_smem_desc(smem_u32(tc_smem), 128u, 256u);
+    const uint64_t descB = umma_smem_desc(smem_u32(tc_smem) + 8192u, 128u, 256u);
+    // instruction descriptor: D = S32 (2 << 4), A = B = signed int8 (1 << 7, 1 << 10), both K-major, N >> 3 at [17,23), M >> 4 at [24,29)
+    const uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((128u >> 4) << 24);
+    for (uint32_t it = 0; it < iters; ++it) {
+      const uint32_t acc = it ? 1u : 0u;
+      asm volatile(
+          "{\n"
+          ".reg .pred p;\n"
+          "setp.ne.b32 p, %4, 0;\n"
+          "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n"
+          "}\n" ::"r"(taddr),
+          "l"(descA), "l"(descB), "r"(idesc), "r"(acc)
+          : "memory");
+    }
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&mbar)) : "memory");
+  }
+  mbar_wait(&mbar, 0u);
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  // read-back: warp w owns TMEM lanes 32w .. 32w+31 (= rows of D), 8 columns per load
+  unsigned int wrong = 0;
+  for (uint32_t c0 = 0; c0 < n; c0 += 8) {
+    uint32_t r[8];
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr + ((32u * warp) << 16) + c0)
+                 : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int j = 0; j < 8; ++j) wrong += r[j] != 32u * iters;
+  }
+  if (wrong) atomicAdd(bad, wrong);
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(256u) : "memory");
+}
+
 }  // namespace
+
+cudaError_t run_tcgen05_peak(uint32_t iters, uint32_t n, int blocks, unsigned int* dBad, double* macsPerLaunch) {
+  static bool attr = false;
+  if (!attr) {
+    cudaError_t e = cudaFuncSetAttribute((const void*)tcgen05_i8_peak_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    attr = true;
+  }
+  tcgen05_i8_peak_kernel<<<blocks, 128, TC_SMEM_BYTES>>>(iters, n, dBad);
+  *macsPerLaunch = (double)blocks * iters * 128.0 * n * 32.0;
+  return cudaGetLastError();
+}
 
 cudaError_t run_l2_copy(const uint4* src, uint4* dst, uint64_t n16, uint32_t iters, int blocks) {
   l2_copy_kernel<<<blocks, BLOCK_THREADS>>>(src, dst, n16, iters);

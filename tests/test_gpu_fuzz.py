@@ -40,7 +40,7 @@ def test_fuzz_single_source():
     t_end, cases = time.time() + 20.0, 0
     while time.time() < t_end or cases < 40:
         n, rp, ci = _graph(rng, small=False)
-        reorder = ["none", "degree", "rcm"][int(rng.integers(0, 3))]
+        reorder = ["none", "degree", "rcm", "jaccard"][int(rng.integers(0, 4))]
         kernel = ["auto", "lazy", "lazy", "eager"][int(rng.integers(0, 4))]
         switching = ["auto", "auto", "auto", "off", "bottom_up", "top_down", "slice"][int(rng.integers(0, 7))]
         with blest.Graph(n, rp, ci, reorder=reorder, kernel=kernel, switching=switching) as g:
@@ -62,7 +62,7 @@ def test_fuzz_multi_source_and_closeness():
     while time.time() < t_end or cases < 24:
         n, rp, ci = _graph(rng, small=True)
         kappa = [32, 64, 128, 256][cases % 4]
-        reorder = ["none", "degree", "rcm"][int(rng.integers(0, 3))]
+        reorder = ["none", "degree", "rcm", "jaccard"][int(rng.integers(0, 4))]
         far_w, reach_w, cc_w, _ = oracle.closeness(n, rp, ci)
         with blest.Graph(n, rp, ci, kappa=kappa, reorder=reorder) as g:
             far = torch.zeros(n, dtype=torch.int64, device="cuda")

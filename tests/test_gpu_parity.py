@@ -126,7 +126,7 @@ def test_contraction_forms_in_traversal(blest, torch_cuda, contraction, kernel):
         check_bfs(blest, torch_cuda, g, graph, sources_for(graph[0], graph[1], 2))
 
 
-@pytest.mark.parametrize("reorder", ["none", "degree", "rcm"])
+@pytest.mark.parametrize("reorder", ["none", "degree", "rcm", "jaccard"])
 @pytest.mark.parametrize("kernel", ["lazy", "eager"])
 def test_reordering_is_invisible(blest, torch_cuda, reorder, kernel):
     for name in ("rmat12", "grid", "union"):

@@ -86,7 +86,7 @@ GRAPHS = {
 
 
 @pytest.mark.parametrize("name", sorted(GRAPHS))
-@pytest.mark.parametrize("reorder", ["none", "degree", "rcm"])
+@pytest.mark.parametrize("reorder", ["none", "degree", "rcm", "jaccard"])
 def test_bvss_roundtrip_and_invariants(name, reorder):
     n, rp, ci = GRAPHS[name]()
     g = blest.Graph(n, rp, ci, host_only=True, reorder=reorder, validate=True)
@@ -192,3 +192,34 @@ def test_build_rejects_bad_input():
     with pytest.raises(blest.BlestError) as e:                   # host-only handles refuse traversal: no CPU fallback
         g.bfs(0, np.zeros(4, np.int32))
     assert e.value.status == binding.EUNSUPPORTED
+
+
+def test_jaccard_with_windows_groups_overlapping_columns():
+    """PAPER.md §4.1 / Alg. 1: columns whose neighbourhoods overlap end up in the same slice set, so masks get denser.
+    Planted case: 64 groups of 8 columns with IDENTICAL neighbourhoods (a complete bipartite block each), ids shuffled.
+    Every group must become exactly one slice set (mask density 8 on those sets); plain degree order cannot do that
+    (all degrees are equal).  On an RMAT graph the density must not drop below the degree order's."""
+    rng = np.random.Generator(np.random.PCG64(11))
+    groups, rows_per = 64, 24
+    n = groups * 8 + groups * rows_per
+    ids = rng.permutation(n)
+    src, dst = [], []
+    for gidx in range(groups):
+        cols = ids[gidx * 8:(gidx + 1) * 8]
+        rows = ids[groups * 8 + gidx * rows_per: groups * 8 + (gidx + 1) * rows_per]
+        for c in cols:
+            src += [c] * rows_per
+            dst += list(rows)
+    n, rp, ci = gg.from_edges(n, np.array(src, np.uint32), np.array(dst, np.uint32))
+    gj = blest.Graph(n, rp, ci, host_only=True, reorder="jaccard")
+    perm = gj.array("perm").astype(np.int64)
+    for gidx in range(groups):
+        cols = ids[gidx * 8:(gidx + 1) * 8]
+        assert len(set(perm[cols] // 8)) == 1, "a group of identical columns was split over slice sets"
+    dj = gj.info().mask_density
+    dd = blest.Graph(n, rp, ci, host_only=True, reorder="degree").info().mask_density
+    assert dj > dd and dj > 3.0
+    n2, rp2, ci2 = gg.rmat(13, 16, 5)
+    d_deg = blest.Graph(n2, rp2, ci2, host_only=True, reorder="degree").info().mask_density
+    d_jac = blest.Graph(n2, rp2, ci2, host_only=True, reorder="jaccard").info().mask_density
+    assert d_jac >= d_deg
