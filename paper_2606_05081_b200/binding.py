@@ -81,11 +81,14 @@ def load(build_if_missing: bool = True):
     global _lib
     if _lib is not None:
         return _lib
-    if build_if_missing:
+    path = _LIB_PATH
+    if os.environ.get("BLEST_DEBUG_LIB") == "1":  # the bounds-asserting build (tests; python -m ...build --debug)
+        path = _build.build_debug() if build_if_missing else _build.LIB_DEBUG
+    elif build_if_missing:
         _build.build()
-    if not os.path.exists(_LIB_PATH):
-        raise ImportError(f"{_LIB_PATH} is missing: run `python -m paper_2606_05081_b200.build` (no CPU fallback exists)")
-    L = ctypes.CDLL(_LIB_PATH)
+    if not os.path.exists(path):
+        raise ImportError(f"{path} is missing: run `python -m paper_2606_05081_b200.build` (no CPU fallback exists)")
+    L = ctypes.CDLL(path)
     vp, u32, u64, i32 = ctypes.c_void_p, ctypes.c_uint32, ctypes.c_uint64, ctypes.c_int
     L.blest_build.argtypes = [ctypes.POINTER(_Csr), ctypes.POINTER(_Options), ctypes.POINTER(vp)]
     L.blest_preprocess_host.argtypes = [ctypes.POINTER(_Csr), ctypes.POINTER(_Options), ctypes.POINTER(vp)]

@@ -21,10 +21,13 @@ NVCC_FLAGS = [
 ]
 
 
-def _stale() -> bool:
-    if not os.path.exists(LIB):
+LIB_DEBUG = os.path.join(HERE, "libblest_debug.so")
+
+
+def _stale(lib: str = LIB) -> bool:
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + HEADERS)
 
 
@@ -36,5 +39,16 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_debug(force: bool = False) -> str:
+    """libblest_debug.so: the same sources with -DBLEST_DEBUG (device-side bounds asserts on every index)."""
+    if force or _stale(LIB_DEBUG):
+        nvcc = os.environ.get("NVCC", "nvcc")
+        subprocess.check_call([nvcc] + NVCC_FLAGS + ["-DBLEST_DEBUG", "-o", LIB_DEBUG] + [os.path.join(CSRC, f) for f in SOURCES])
+    return LIB_DEBUG
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--debug" in sys.argv:
+        print(build_debug(force="--force" in sys.argv))
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -600,6 +600,7 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
   const bool devOut = is_device_ptr(levels_out);
   BfsParams p{};
   p.n = h->n; p.Ns = h->Ns; p.nwords = h->nwords; p.qcap = h->qcap; p.nnz = h->nnz;
+  p.nQuads = h->nQuads; p.wlCap = h->nSweepWords + 16384u;
   p.setPtr = h->dSetPtr; p.rowIds = reinterpret_cast<const uint4*>(h->dRowIds); p.masks = h->dMasks;
   p.rowptr = h->dRowptr; p.colidx = h->dColidx;
   p.perm = h->hasPerm ? h->dPerm : nullptr;
@@ -731,7 +732,7 @@ static int ensure_ms_workspace(blest_graph* g) {
 }
 
 static void fill_ms_params(blest_graph* h, MsParams& p) {
-  p.n = h->n; p.Ns = h->Ns; p.rho = h->rho; p.qcap = h->qcap;
+  p.n = h->n; p.Ns = h->Ns; p.rho = h->rho; p.qcap = h->qcap; p.nQuads = h->nQuads;
   p.setPtr = h->dSetPtr; p.rowIds = reinterpret_cast<const uint4*>(h->dRowIds); p.masks = h->dMasks;
   p.perm = h->hasPerm ? h->dPerm : nullptr;
   p.iperm = h->hasPerm ? h->dIperm : nullptr;

@@ -74,8 +74,10 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_eager_kernel(const __gri
     BigSeg* bigList = sh.bigList[warp];
     uint32_t* bigCnt = &sh.bigCnt[warp];
     for (uint32_t i = gwarp; i < qcount; i += nwarps) {
+      BLEST_ASSERT(i < p.qcap);
       const uint2 e = Qc[i];
       const uint32_t nq = (e.y & 31u) + 1u, s = e.y >> 5;
+      BLEST_ASSERT(s < p.Ns && (uint64_t)e.x + nq <= p.nQuads);
       uint4 rows = make_uint4(0, 0, 0, 0);
       uint32_t m = 0;
       if (lane < nq) {
@@ -97,6 +99,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_eager_kernel(const __gri
         lu[c] = 0;
         sa[c] = sb[c] = 0;
         if ((hits >> c) & 1u) {
+          BLEST_ASSERT(ru[c] < p.n);
           lu[c] = p.L[ru[c]];
           sa[c] = __ldg(&p.setPtr[ru[c] >> 3]);
           sb[c] = __ldg(&p.setPtr[(ru[c] >> 3) + 1]);
@@ -125,6 +128,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_eager_kernel(const __gri
         ok = tot == 0u || (uint64_t)first + tot <= p.qcap;
         if (!ok && lane == 0) report_overflow(ctrl, p.hostStatus);
       }
+      BLEST_ASSERT(!ok || cnt == 0u || (uint64_t)pos + cnt <= p.qcap);
       if (ok)
         for (uint32_t k = 0; k < nseg; ++k) emit_segment(Qn, pos, 0, segA[k], segN[k], segS[k], bigList, bigCnt);
       flush_big_segments(Qn, bigList, bigCnt, lane);

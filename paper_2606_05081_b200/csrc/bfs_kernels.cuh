@@ -15,6 +15,8 @@ struct BfsParams {
   // graph (immutable during traversal)
   uint32_t n, Ns, nwords, qcap;
   uint64_t nnz;
+  uint64_t nQuads;         // quads stored (bounds of rowIds / masks; debug asserts)
+  uint32_t wlCap;          // capacity of a frontier word list (debug asserts)
   const uint32_t* setPtr;  // Ns+1 quad offsets
   const uint4* rowIds;     // nQuads
   const uint32_t* masks;   // nQuads
@@ -65,6 +67,7 @@ struct BfsParams {
 
 struct MsParams {
   uint32_t n, Ns, rho, qcap;
+  uint64_t nQuads;  // bounds of rowIds / masks (debug asserts)
   const uint32_t* setPtr;
   const uint4* rowIds;
   const uint32_t* masks;

@@ -103,6 +103,7 @@ __device__ __forceinline__ uint32_t wl_reserve(LazyShared& sh, unsigned int* wlc
   return 0x80000000u | atomicAdd(wlc, cnt);
 }
 __device__ __forceinline__ void wl_store(LazyShared& sh, uint32_t* WLn, uint32_t slot, uint32_t w) {
+  BLEST_ASSERT((slot & 0x80000000u) || slot < WL_STAGE);
   if (slot & 0x80000000u) WLn[slot & 0x7FFFFFFFu] = w;
   else sh.wl[slot] = w;
 }
@@ -138,11 +139,14 @@ struct Marks {
   bool probeFn;
   uint32_t* hub;
   uint32_t hubLimit;  // HUB_BITS, or 0 = filter off (graphs that are not degree-sorted: low ids are no hubs there)
+  uint32_t nBits;     // vertices (bound of every mark; debug asserts)
 };
 template <int U>
 __device__ __forceinline__ void mark_batch(const Marks& mk, const uint32_t (&v)[U], uint32_t valid) {
   const uint32_t* V = mk.V;
   uint32_t* Fn = mk.Fn;
+#pragma unroll
+  for (int j = 0; j < U; ++j) BLEST_ASSERT(!((valid >> j) & 1u) || v[j] < mk.nBits);
 #pragma unroll
   for (int j = 0; j < U; ++j)
     if (((valid >> j) & 1u) && v[j] < mk.hubLimit) {
@@ -195,6 +199,7 @@ __device__ __forceinline__ void expand_edges(const BfsParams& p, const Marks& Fn
       const uint32_t bp = __shfl_sync(FULL, basePtr, own);
       v[j] = 0;
       if (idx < total) {
+        BLEST_ASSERT((uint64_t)bp + idx < p.nnz);
         v[j] = __ldcs(p.colidx + (bp + idx));
         valid |= 1u << j;
       }
@@ -212,6 +217,7 @@ __device__ __forceinline__ void warp_edges(const BfsParams& p, const Marks& Fn, 
       const uint32_t idx = base + 32u * j + lane;
       v[j] = 0;
       if (idx < e1) {
+        BLEST_ASSERT(idx < p.nnz);
         v[j] = __ldcs(p.colidx + idx);
         valid |= 1u << j;
       }
@@ -240,6 +246,7 @@ __device__ __forceinline__ void warp_slices(const BfsParams& p, const Marks& Fn,
       r[k] = make_uint4(0, 0, 0, 0);
       m[k] = 0;
       if (idx < nq) {
+        BLEST_ASSERT((uint64_t)a + idx < p.nQuads);
         r[k] = __ldcs(p.rowIds + a + idx);
         m[k] = __ldcs(p.masks + a + idx);
       }
@@ -275,6 +282,7 @@ __device__ __forceinline__ void expand_slices(const BfsParams& p, const Marks& F
       r[j] = make_uint4(0, 0, 0, 0);
       m[j] = 0;
       if (ok[j]) {
+        BLEST_ASSERT((uint64_t)bp + idx < p.nQuads);
         r[j] = __ldcs(p.rowIds + (bp + idx));
         m[j] = __ldcs(p.masks + (bp + idx));
       }
@@ -303,6 +311,7 @@ __device__ __forceinline__ void emit_chunks(const BfsParams& p, Ctrl* ctrl, uint
     if (lane == 0) report_overflow(ctrl, p.hostStatus);
     return;
   }
+  BLEST_ASSERT((uint64_t)pos + nent <= p.chunkCap);
   for (uint32_t i = lane; i < nent; i += 32) p.chunks[pos + i] = make_uint4(start + i * per, min(per, count - i * per), alpha, type);
 }
 
@@ -326,6 +335,7 @@ __device__ __forceinline__ void td_phase_a(const BfsParams& p, LazyShared& sh, c
     uint32_t t = NONE, fw = 0, thr = 0x9999u;
     if (lane < W && i < wlCount) t = __ldcg(&WLc[i]);
     if (t != NONE) {  // NONE: staging sentinel (wl_reserve)
+      BLEST_ASSERT(t < p.nSweepWords);
       fw = Fp[t];
       if (sw == 0 || sw == 5) thr = __ldg(&p.popThr[t]);
     }
@@ -413,6 +423,7 @@ __device__ __forceinline__ void td_phase_b(const BfsParams& p, uint32_t nChunks,
   const uint32_t lane = threadIdx.x & 31;
   const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
   for (uint32_t i = gwarp; i < nChunks; i += nwarps) {
+    BLEST_ASSERT(i < p.chunkCap);
     const uint4 e = __ldcg(&p.chunks[i]);
     if (e.w) warp_edges(p, Fn, e.x, e.x + e.y, lane);
     else warp_slices<CONTR>(p, Fn, e.x, e.y, e.z, lane);
@@ -444,8 +455,10 @@ __device__ __forceinline__ void write_levels_dense(const BfsParams& p, uint32_t 
 #pragma unroll
     for (int q = 0; q < 8; ++q) c.mf += dg[q];
 #pragma unroll
-    for (int q = 0; q < 8; ++q)
+    for (int q = 0; q < 8; ++q) {
+      BLEST_ASSERT(!((on >> q) & 1u) || (o[q] < p.n && u[q] < p.n));
       if ((on >> q) & 1u) p.lvl[o[q]] = level;
+    }
   }
 }
 // Same for a lane's own sparse word (a few bits): four vertices in flight.
@@ -470,8 +483,10 @@ __device__ __forceinline__ void write_levels_sparse(const BfsParams& p, uint32_t
 #pragma unroll
     for (int q = 0; q < 4; ++q) c.mf += dg[q];
 #pragma unroll
-    for (int q = 0; q < 4; ++q)
+    for (int q = 0; q < 4; ++q) {
+      BLEST_ASSERT(!on[q] || (o[q] < p.n && u[q] < p.n));
       if (on[q]) p.lvl[o[q]] = level;
+    }
   }
 }
 
@@ -498,8 +513,10 @@ __device__ __forceinline__ void write_levels_list(const BfsParams& p, const uint
   for (int q = 0; q < 8; ++q) sum += dg[q];
   c.mf += sum;
 #pragma unroll
-  for (int q = 0; q < 8; ++q)
+  for (int q = 0; q < 8; ++q) {
+    BLEST_ASSERT(!((on >> q) & 1u) || (o[q] < p.n && u[q] < p.n));
     if ((on >> q) & 1u) p.lvl[o[q]] = level;
+  }
 }
 
 // Stage 2 after a top-down Stage 1: frontier finalisation (readings R9/R10).
@@ -544,6 +561,7 @@ __device__ __forceinline__ void td_finalize(const BfsParams& p, LazyShared& sh, 
       }
       base = __shfl_sync(FULL, base, 0);
       if (base + nd <= DLIST_CAP) {
+        BLEST_ASSERT(!dense || base + __popc(dmask & ((1u << lane) - 1u)) < DLIST_CAP);
         if (dense) sh.dlist[base + __popc(dmask & ((1u << lane) - 1u))] = make_uint2(t, fm);
       } else {
         write_levels_dense(p, wb, fm, dmask, (int32_t)level, lane, c);  // pool full: the owner does them itself
@@ -583,6 +601,7 @@ __device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_
     if (u[k] != NONE) {
       if (!DEFER && (u[k] & CSR_STAGE)) staged |= 1u << k;
       else {
+        BLEST_ASSERT(u[k] < p.n);
         h[k] = __ldcs(&p.head[u[k]]);
         act |= 1u << k;
       }
@@ -633,6 +652,7 @@ __device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_
 #pragma unroll
     for (int k = 0; k < K; ++k)
       if ((more >> k) & 1u) {
+        BLEST_ASSERT(listCount + pos[k] < BU_LIST);
         list[listCount + pos[k]] = u[k] | CSR_STAGE;
         prefetch_l2(&p.rowptr[u[k]]);
       }
@@ -664,6 +684,7 @@ __device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_
     while (!f && ptr < stop) {  // four neighbours per step
       uint32_t v[4], fwd[4];
       const uint32_t cnt = min(4u, stop - ptr);
+      BLEST_ASSERT((uint64_t)ptr + cnt <= p.nnz);
 #pragma unroll
       for (int j = 0; j < 4; ++j) v[j] = (uint32_t)j < cnt ? __ldg(&p.colidx[ptr + j]) : 0u;
 #pragma unroll
@@ -752,6 +773,7 @@ __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uin
       oldF[k] = 1u;
       if ((found >> k) & 1u) {
         const uint32_t uu = u[k] & ~CSR_STAGE, bit = 1u << (uu & 31u);
+        BLEST_ASSERT(o[k] < p.n && uu < p.n);
         p.lvl[o[k]] = (int32_t)level;
         atomicOr(&p.V[uu >> 5], bit);
         oldF[k] = atomicOr(&Fn[uu >> 5], bit);
@@ -805,6 +827,7 @@ __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uin
         }
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
+          BLEST_ASSERT(!((found >> k) & 1u) || (o[k] < p.n && u[k] < p.n));
           if ((found >> k) & 1u) p.lvl[o[k]] = (int32_t)level;  // lane = bit: coalesced when there is no reordering
           const uint32_t fmk = __ballot_sync(FULL, (found >> k) & 1u);
           if (lane == 8u * sub + k) fmw = fmk;
@@ -833,6 +856,7 @@ __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uin
       uint32_t at = listCount + incl - cnt;
       for (uint32_t bits = unvw; bits; bits &= bits - 1) {
         const uint32_t u = myw * 32u + (uint32_t)(__ffs(bits) - 1);
+        BLEST_ASSERT(at < BU_LIST && u < p.n);
         list[at++] = u;
         prefetch_l2(&p.head[u]);
       }
@@ -989,6 +1013,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
           dg = __ldg(&p.deg[v]);
           atomicOr(&p.V[v >> 5], bit);
         }
+        BLEST_ASSERT(!disc || (o < p.n && v < p.n));
         if (disc) p.lvl[o] = 1;
         c.mf += dg;
         c.nnew += disc ? 1u : 0u;
@@ -1008,7 +1033,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       grid_barrier(&ctrl->bar, epoch);
       if (leader) tStage1 = globaltimer();
     } else {
-      const Marks mk{p.V, Fn, p.hubFilter || mf > 4ull * nu, sh.hub, p.hubFilter ? HUB_BITS : 0u};
+      const Marks mk{p.V, Fn, p.hubFilter || mf > 4ull * nu, sh.hub, p.hubFilter ? HUB_BITS : 0u, p.n};
       if (p.hubFilter) {
         for (uint32_t i = threadIdx.x; i < HUB_BITS / 32; i += blockDim.x) sh.hub[i] = 0;
         __syncthreads();

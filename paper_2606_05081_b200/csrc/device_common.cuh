@@ -1,10 +1,20 @@
 // device_common.cuh -- shared device-side pieces of the BLEST kernels: control block, grid barrier, work-queue
 // entry encoding, warp-aggregated queue expansion, slice x frontier-word contraction forms.
 #pragma once
+#include <cassert>
 #include <cstdint>
 #include <cuda_runtime.h>
 
 #include "../../include/blest.h"
+
+// Debug build (python -m paper_2606_05081_b200.build --debug -> libblest_debug.so, -DBLEST_DEBUG): every queue / list /
+// chunk / bitmap / graph-array index of the kernels is bounds-checked with a device assert (compute-sanitizer is closed on
+// this GPU pool; tests/test_gpu_parity.py runs the small-graph suite against this build).
+#ifdef BLEST_DEBUG
+#define BLEST_ASSERT(cond) assert(cond)
+#else
+#define BLEST_ASSERT(cond) ((void)0)
+#endif
 
 namespace blest {
 
@@ -144,6 +154,7 @@ __device__ __forceinline__ uint32_t seg_entries(uint32_t type, uint32_t count) {
 }
 __device__ __forceinline__ void write_entry(uint2* Q, uint32_t pos, uint32_t type, uint32_t start, uint32_t count,
                                             uint32_t s, uint32_t i) {
+  BLEST_ASSERT(i < seg_entries(type, count));
   if (type) Q[pos + i] = make_edge_entry(start + i * TD_CHUNK, min(TD_CHUNK, count - i * TD_CHUNK));
   else Q[pos + i] = make_slice_entry(start + i * VSS_QUADS, min(VSS_QUADS, count - i * VSS_QUADS), s);
 }

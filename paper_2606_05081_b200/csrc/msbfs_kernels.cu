@@ -73,8 +73,10 @@ __device__ __forceinline__ void ms_stage1(const MsParams& p, MsShared& sh, const
   const uint32_t lane = threadIdx.x & 31;
   const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
   for (uint32_t i = gwarp; i < qcount; i += nwarps) {
+    BLEST_ASSERT(i < p.qcap);
     const uint2 e = Qc[i];
     const uint32_t nq = (e.y & 31u) + 1u, s = e.y >> 5;
+    BLEST_ASSERT(s < p.Ns && (uint64_t)e.x + nq <= p.nQuads);
     uint4 rows = make_uint4(0, 0, 0, 0);
     uint32_t m = 0;
     if (lane < nq) {
@@ -106,6 +108,7 @@ __device__ __forceinline__ void ms_stage1(const MsParams& p, MsShared& sh, const
           for (int w = 0; w < KW; ++w) M[w] |= fset[j * KW + w];
         }
         const uint32_t u = ru[c];
+        BLEST_ASSERT(u < p.n);
         const uint64_t idx = (uint64_t)(u & 7u) * p.rho + (u >> 3);  // getVI(u, rho)
         uint32_t any = 0;
 #pragma unroll
@@ -135,14 +138,19 @@ __device__ __forceinline__ void ms_stage1(const MsParams& p, MsShared& sh, const
   }
 }
 
-template <int KW>
+// PS: per-source counts (a source subset, reading R13) instead of the paper's target-side sums; a separate
+// instantiation, so that its counters cost the all-vertices kernel no registers.
+template <int KW, bool PS>
 __device__ __forceinline__ void ms_stage2(const MsParams& p, MsShared& sh, uint32_t level, uint64_t b0, uint32_t nb,
                                           uint2* Qn, uint32_t tBase) {
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + warp, nwarps = gridDim.x * WARPS_PER_BLOCK;
   BigSeg* bigList = sh.bigList[warp];
   uint32_t* bigCnt = &sh.bigCnt[warp];
-  const bool perSource = (p.farS != nullptr) || (p.reachS != nullptr);
+  constexpr bool perSource = PS;
+  uint32_t pacc[KW];  // per-source counts of this sweep kept by lane c mod 32 for instance c = 32 w + lane
+#pragma unroll
+  for (int w = 0; w < KW; ++w) pacc[w] = 0;
   for (uint64_t sb = (uint64_t)gwarp * 32; sb < p.Ns; sb += (uint64_t)nwarps * 32) {
     const uint32_t s = (uint32_t)sb + lane;  // consecutive threads -> consecutive slice sets
     uint32_t cnt = 0, a = 0, nq = 0;
@@ -151,8 +159,10 @@ __device__ __forceinline__ void ms_stage2(const MsParams& p, MsShared& sh, uint3
       const uint32_t nd = __popc(__ballot_sync(0xffffffffu, isDirty));
       if (lane == 0) sh.cnt[warp][4] += nd;
     }
-    if (isDirty) {  // skip slice sets nobody marked
-      p.dirty[s] = 0;
+    // skip slice sets nobody marked.  With per-source counts the block is entered by the whole warp as
+    // soon as one lane's set is dirty (clean lanes carry zero words), so that the counting below is warp-uniform.
+    if (perSource ? __any_sync(0xffffffffu, isDirty) : isDirty) {
+      if (isDirty) p.dirty[s] = 0;
       uint32_t A = 0;
       constexpr uint32_t R = KW <= 2 ? 8u : (KW == 4 ? 4u : 2u);  // rows whose words are in flight together
 #pragma unroll
@@ -161,8 +171,13 @@ __device__ __forceinline__ void ms_stage2(const MsParams& p, MsShared& sh, uint3
 #pragma unroll
         for (uint32_t r = 0; r < R; ++r) {
           const uint64_t idx = (uint64_t)(j0 + r) * p.rho + s;
-          load_words<KW>(p.Vn, idx, nx[r]);
-          load_words<KW>(p.Vc, idx, cu[r]);
+          if (isDirty) {
+            load_words<KW>(p.Vn, idx, nx[r]);
+            load_words<KW>(p.Vc, idx, cu[r]);
+          } else {
+#pragma unroll
+            for (int w = 0; w < KW; ++w) nx[r][w] = cu[r][w] = 0;
+          }
         }
 #pragma unroll
         for (uint32_t r = 0; r < R; ++r) {
@@ -175,19 +190,40 @@ __device__ __forceinline__ void ms_stage2(const MsParams& p, MsShared& sh, uint3
             any |= diff[w];
             pc += __popc(diff[w]);
           }
-          store_words<KW>(p.F, idx, diff);  // PAPER.md:610 (unconditional)
+          if (isDirty) store_words<KW>(p.F, idx, diff);  // PAPER.md:610 (unconditional for a swept set)
+          if (perSource) {
+            // Per-source counts (reading R13) = a positional popcount over the vertices: how many of the warp's 32 rows
+            // have bit c set, for every instance c.  Few bits: one shared-memory atomic each.  Many (the dense middle
+            // levels, where those atomics would pile up on kappa addresses): bit-sliced, one ballot per instance, the
+            // count kept by lane c mod 32 in a register.
+            const uint32_t tot = __reduce_add_sync(0xffffffffu, pc);
+            if (tot > 32u) {
+#pragma unroll
+              for (int w = 0; w < KW; ++w) {
+#pragma unroll 8
+                for (uint32_t b = 0; b < 32u; ++b) {
+                  const uint32_t k = (uint32_t)__popc(__ballot_sync(0xffffffffu, (diff[w] >> b) & 1u));
+                  if (lane == b) pacc[w] += k;
+                }
+              }
+            } else if (any) {
+#pragma unroll
+              for (int w = 0; w < KW; ++w)
+                for (uint32_t d = diff[w]; d; d &= d - 1) atomicAdd(&sh.perSource[w * 32u + (__ffs(d) - 1)], 1u);
+            }
+          }
           if (any) {
             store_words<KW>(p.Vc, idx, nx[r]);
             A |= any;
-            if (perSource || p.levels) {
+            if (p.levels) {
               const uint32_t u = s * 8u + j;
               const uint32_t uo = p.iperm ? __ldg(&p.iperm[u]) : u;
 #pragma unroll
               for (int w = 0; w < KW; ++w)
                 for (uint32_t d = diff[w]; d; d &= d - 1) {
                   const uint32_t c = w * 32u + (__ffs(d) - 1);
-                  if (perSource) atomicAdd(&sh.perSource[c], 1u);
-                  if (p.levels) p.levels[(b0 + c) * (uint64_t)p.n + uo] = (int32_t)level;
+                  BLEST_ASSERT(c < nb && uo < p.n);
+                  p.levels[(b0 + c) * (uint64_t)p.n + uo] = (int32_t)level;
                 }
             }
             if (p.farT) p.farT[idx] += (unsigned long long)level * pc;  // Eq. 7: far[idx] += l * popc(diff)
@@ -210,8 +246,14 @@ __device__ __forceinline__ void ms_stage2(const MsParams& p, MsShared& sh, uint3
       ok = tot == 0u || (uint64_t)first + tot <= p.qcap;
       if (!ok && lane == 0) report_overflow(p.ctrl, p.hostStatus);
     }
+    BLEST_ASSERT(!(cnt && ok) || (uint64_t)pos + cnt <= p.qcap);
     if (cnt && ok) emit_segment(Qn, pos, 0, a, nq, s, bigList, bigCnt);
     flush_big_segments(Qn, bigList, bigCnt, lane);
+  }
+  if (perSource) {
+#pragma unroll
+    for (int w = 0; w < KW; ++w)
+      if (pacc[w]) atomicAdd(&sh.perSource[w * 32u + lane], pacc[w]);
   }
   __syncthreads();
   if (perSource && threadIdx.x < nb) {
@@ -226,7 +268,7 @@ __device__ __forceinline__ void ms_stage2(const MsParams& p, MsShared& sh, uint3
   __syncthreads();
 }
 
-template <int KW>
+template <int KW, bool PS>
 __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_constant__ MsParams p) {
   __shared__ MsShared sh;
   constexpr uint32_t KAPPA = 32u * KW;
@@ -262,7 +304,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_co
     }
     grid_barrier(&ctrl->bar, epoch);
     // level 0 = the finalisation sweep over the sources themselves (far += 0, reach += 1, level 0, enqueue their sets)
-    ms_stage2<KW>(p, sh, 0, b0, nb, p.Q[1], tEnd);
+    ms_stage2<KW, PS>(p, sh, 0, b0, nb, p.Q[1], tEnd);
     {
       const uint32_t t = grid_barrier_tail(&ctrl->bar, epoch, &sh.tailSlot);
       tStart = tEnd;
@@ -277,7 +319,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_co
       ++nLevels;
       ms_stage1<KW>(p, sh, p.Q[par], qcount);
       grid_barrier(&ctrl->bar, epoch);
-      ms_stage2<KW>(p, sh, level, b0, nb, p.Q[par ^ 1u], tEnd);
+      ms_stage2<KW, PS>(p, sh, level, b0, nb, p.Q[par ^ 1u], tEnd);
       const uint32_t t = grid_barrier_tail(&ctrl->bar, epoch, &sh.tailSlot);
       tStart = tEnd;
       tEnd = t;
@@ -332,11 +374,12 @@ int coop_blocks(K kernel) {
 cudaError_t launch_msbfs(const MsParams& p, int gridBlocks, cudaStream_t st) {
   void* args[] = {(void*)&p};
   const void* k = nullptr;
+  const bool ps = p.farS != nullptr || p.reachS != nullptr;
   switch (p.kappa) {
-    case 32: k = (const void*)msbfs_kernel<1>; break;
-    case 64: k = (const void*)msbfs_kernel<2>; break;
-    case 128: k = (const void*)msbfs_kernel<4>; break;
-    case 256: k = (const void*)msbfs_kernel<8>; break;
+    case 32: k = ps ? (const void*)msbfs_kernel<1, true> : (const void*)msbfs_kernel<1, false>; break;
+    case 64: k = ps ? (const void*)msbfs_kernel<2, true> : (const void*)msbfs_kernel<2, false>; break;
+    case 128: k = ps ? (const void*)msbfs_kernel<4, true> : (const void*)msbfs_kernel<4, false>; break;
+    case 256: k = ps ? (const void*)msbfs_kernel<8, true> : (const void*)msbfs_kernel<8, false>; break;
     default: return cudaErrorInvalidValue;
   }
   return cudaLaunchCooperativeKernel(k, dim3(gridBlocks), dim3(BLOCK_THREADS), args, 0, st);
@@ -353,6 +396,9 @@ cudaError_t launch_closeness_finalize(uint32_t n, uint32_t rho, const uint32_t* 
   return cudaGetLastError();
 }
 
-int max_coop_blocks_msbfs() { return std::min(coop_blocks(msbfs_kernel<4>), coop_blocks(msbfs_kernel<8>)); }
+int max_coop_blocks_msbfs() {
+  return std::min(std::min(coop_blocks(msbfs_kernel<4, false>), coop_blocks(msbfs_kernel<8, false>)),
+                  std::min(coop_blocks(msbfs_kernel<4, true>), coop_blocks(msbfs_kernel<8, true>)));
+}
 
 }  // namespace blest

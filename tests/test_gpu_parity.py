@@ -431,3 +431,55 @@ def test_microbenchmarks_run(blest, torch_cuda):
     assert blest.l2_microbench(32 << 20, 10) > 500.0          # GB/s, L2-resident copy
     assert 200.0 < blest.barrier_microbench(500) < 20000.0     # ns per grid barrier
     assert blest.mma_microbench("mma_u8", 256)[0] > 10.0
+
+
+def test_small_graph_suite_under_bounds_asserts():
+    """compute-sanitizer is closed on this GPU pool, so the kernels carry their own bounds checks: libblest_debug.so is
+    the same source with -DBLEST_DEBUG (a device assert on every queue / list / chunk / bitmap / graph-array index).
+    The small and degenerate graphs go through every kernel, forced path, reordering and kappa against it, in a
+    subprocess (the library is chosen when it is first loaded); a tripped assert kills the context and fails the run."""
+    import os
+    import subprocess
+    import sys
+
+    code = (
+        "import numpy as np, torch, graphgen as gg, oracle, paper_2606_05081_b200 as blest\n"
+        "from paper_2606_05081_b200 import binding\n"
+        "assert binding.load()._name.endswith('libblest_debug.so')\n"
+        "makers = [lambda: gg.path(1000), lambda: gg.star(5000, 17), lambda: gg.complete(130), lambda: gg.gnm(1003, 2500, 7),\n"
+        "          lambda: gg.disjoint_union(gg.path(9), gg.empty(5), gg.complete(6), gg.cycle(11)), lambda: gg.grid2d(37, 41, 0.05, 8),\n"
+        "          lambda: gg.rmat(12, 16, 9), lambda: gg.path(2), lambda: gg.empty(1), lambda: gg.rmat(15, 16, 4)]\n"
+        "opts = [dict(kernel='lazy'), dict(kernel='lazy', reorder='degree'), dict(kernel='lazy', reorder='rcm', persist_l2=False),\n"
+        "        dict(kernel='lazy', switching='off'), dict(kernel='lazy', switching='bottom_up'), dict(kernel='lazy', switching='top_down'),\n"
+        "        dict(kernel='lazy', switching='slice', contraction='mma_b1'), dict(kernel='eager'), dict(kernel='eager', reorder='jaccard')]\n"
+        "cases = 0\n"
+        "for mk in makers:\n"
+        "    n, rp, ci = mk()\n"
+        "    srcs = sorted({0, n - 1, int(np.argmax(gg.degrees(rp)))})\n"
+        "    for o in opts:\n"
+        "        with blest.Graph(n, rp, ci, **o) as g:\n"
+        "            out = torch.empty(n, dtype=torch.int32, device='cuda')\n"
+        "            for s in srcs:\n"
+        "                g.bfs(s, out)\n"
+        "                assert np.array_equal(out.cpu().numpy(), oracle.bfs(n, rp, ci, s)), (o, s)\n"
+        "            assert g.last_status() == 0\n"
+        "            cases += 1\n"
+        "    if n <= 5000:\n"
+        "        for kappa in (32, 64, 128, 256):\n"
+        "            with blest.Graph(n, rp, ci, kappa=kappa, reorder='degree') as g:\n"
+        "                cc = torch.zeros(n, dtype=torch.float64, device='cuda')\n"
+        "                g.closeness(cc)\n"
+        "                assert np.array_equal(cc.cpu().numpy(), oracle.closeness(n, rp, ci)[2])\n"
+        "                k = min(n, kappa + 3)\n"
+        "                ms = np.arange(k, dtype=np.uint32)\n"
+        "                lv = torch.empty((k, n), dtype=torch.int32, device='cuda')\n"
+        "                g.msbfs(ms, lv)\n"
+        "                assert np.array_equal(lv.cpu().numpy(), oracle.msbfs(n, rp, ci, ms))\n"
+        "                assert g.last_status() == 0\n"
+        "                cases += 1\n"
+        "print('debug build ok', cases)\n"
+    )
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, BLEST_DEBUG_LIB="1", PYTHONPATH=root)
+    r = subprocess.run([sys.executable, "-c", code], env=env, cwd=root, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0 and "debug build ok" in r.stdout, (r.stdout[-500:], r.stderr[-2000:])

@@ -57,3 +57,26 @@ def test_sources():
     s = gg.pick_sources(rp, 64, 6)
     assert s.size == 64 and np.unique(s).size == 64 and np.all(gg.degrees(rp)[s] > 0)
     assert np.array_equal(s, gg.pick_sources(rp, 64, 6))
+
+
+def test_rmat_quadrant_probabilities_at_every_bit_level():
+    """BASELINE.json configs: Graph500 parameters (a, b, c, d) = (0.57, 0.19, 0.19, 0.05) at EVERY one of the `scale`
+    recursion levels.  The raw edge list (no relabelling, before clean-up) is drawn directly from the generator and
+    the quadrant of each endpoint-bit pair is counted per level; each frequency must sit within 5 standard errors."""
+    import ctypes
+
+    scale, m = 14, 1 << 18
+    L = gg._load()
+    src = np.empty(m, dtype=np.uint32)
+    dst = np.empty(m, dtype=np.uint32)
+    L.gg_rmat_edges(scale, m, 4242, 0.57, 0.19, 0.19, None, gg._p(src), gg._p(dst))
+    want = np.array([0.57, 0.19, 0.19, 0.05])
+    for lvl in range(scale):
+        ub = (src >> lvl) & 1
+        vb = (dst >> lvl) & 1
+        freq = np.bincount((ub * 2 + vb).astype(np.int64), minlength=4) / m      # quadrant = (row bit, column bit)
+        se = np.sqrt(want * (1 - want) / m)
+        assert np.all(np.abs(freq - want) < 5 * se), (lvl, freq)
+    # the levels are independent draws: the joint frequency of (a at level 0, a at level 1) is a * a
+    both = np.mean((((src | dst) & 3) == 0))
+    assert abs(both - 0.57 * 0.57) < 5 * np.sqrt(0.3249 * 0.6751 / m)
