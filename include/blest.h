@@ -90,6 +90,10 @@ typedef struct {
                       Result-neutral; not part of the paper's method. */
   uint32_t queue_capacity; /* 0 auto (exact bounds) | entries: caps the work queues / chunk list (tests of the
                       overflow report) */
+  int tune[4];     /* experiment switches of the kernels, 0 = default: [0] = 1: the balanced top-down phase stages its
+                      slice tiles in shared memory with TMA bulk copies (cp.async.bulk + mbarrier, two stages per warp)
+                      instead of 128-bit loads into registers -- measured 14 % slower on config 4, hence off by default
+                      (DESIGN.md §6); [1..3] unused */
   int reserved[6]; /* [0]: switching == 5 ("scripted", tests): level l runs bottom-up iff bit min(l,31) is set;
                       [1..5]: tuning overrides of the switch cost model in 0.01 ps per unit (top-down edge, top-down
                       vertex, bottom-up vertex, bottom-up scanned neighbour, bottom-up bitmap word); 0 = default */

@@ -44,7 +44,7 @@ class _Options(ctypes.Structure):
                 ("kernel", ctypes.c_int), ("switching", ctypes.c_int), ("contraction", ctypes.c_int),
                 ("kappa", ctypes.c_int), ("trace", ctypes.c_int), ("eta", ctypes.c_float), ("gamma", ctypes.c_float),
                 ("persist_l2", ctypes.c_int), ("prune_components", ctypes.c_int), ("queue_capacity", ctypes.c_uint32),
-                ("reserved", ctypes.c_int * 6)]
+                ("tune", ctypes.c_int * 4), ("reserved", ctypes.c_int * 6)]
 
 
 class _Info(ctypes.Structure):
@@ -153,7 +153,7 @@ def _stream(stream):
 
 def _options(reorder="none", builder=0, validate=False, kernel="auto", switching="auto", contraction="auto", kappa=64,
              trace=True, eta=0.0, gamma=0.0, bu_mask=0, costs=None, persist_l2=True, prune_components=True,
-             queue_capacity=0) -> _Options:
+             queue_capacity=0, tma_tiles=False) -> _Options:
     o = _Options()
     o.reorder = REORDER[reorder] if isinstance(reorder, str) else int(reorder)
     o.builder = int(builder)
@@ -168,6 +168,7 @@ def _options(reorder="none", builder=0, validate=False, kernel="auto", switching
     o.persist_l2 = 0 if persist_l2 else 1
     o.prune_components = 0 if prune_components else 1
     o.queue_capacity = int(queue_capacity)
+    o.tune[0] = int(bool(tma_tiles))
     o.reserved[0] = int(bu_mask)
     for k, c in enumerate(costs or ()):  # switch cost model overrides, ps per unit (tuning only): td_edge, td_vertex,
         o.reserved[1 + k] = int(round(100 * float(c)))  # bu_vertex, bu_scan, bu_word

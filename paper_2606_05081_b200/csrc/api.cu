@@ -638,6 +638,7 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
   p.switching = h->opt.switching;
   p.contraction = h->opt.contraction ? h->opt.contraction : 1;  // auto -> ALU (measured fastest)
   p.buMask = (uint32_t)h->opt.reserved[0];
+  p.tmaTiles = h->opt.tune[0] == 1;
   p.eta = h->opt.eta;
   p.gamma = h->opt.gamma;
   if ((h->isoBits[p.src >> 5] >> (p.src & 31u)) & 1u) {

@@ -61,6 +61,7 @@ struct BfsParams {
   float eta, gamma;
   // switch cost model, picoseconds per unit
   float cTdEdge, cTdNew, cTdVertex, cTdWord, cBuVertex, cBuScan, cBuWord;
+  int tmaTiles;   // balanced top-down phase: slice tiles staged by TMA bulk copies (options.tune[0])
   int hubFilter;  // top-down marks of low-id vertices are de-duplicated per CTA (degree-sorted graphs)
   float scanExp;  // exponent of nnz/mf in the estimate of neighbours examined per bottom-up vertex
 };

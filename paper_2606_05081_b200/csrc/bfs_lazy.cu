@@ -35,6 +35,7 @@ constexpr uint32_t NONE = 0xffffffffu;
 constexpr uint32_t BU_LIST = 512;   // per-warp list of unvisited vertices (sparse bottom-up groups)
 constexpr uint32_t BU_BATCH = 256;  // vertices per bottom-up batch: 8 per lane in flight
 constexpr uint32_t DLIST_CAP = 1024;  // finalisation: dense words a CTA pools before its warps share them
+constexpr uint32_t TILE_QUADS = 64;  // balanced top-down phase: quads per TMA-staged slice tile (1 KB of row ids + 256 B of masks)
 constexpr uint32_t HUB_BITS = 1u << 17;  // top-down: marks of the first 2^17 vertices are de-duplicated per CTA in shared memory
 
 struct LazyShared {
@@ -42,10 +43,22 @@ struct LazyShared {
   unsigned long long ctl[4];  // control words of the level, read by one thread and broadcast
   uint32_t wlCnt;
   uint32_t wlBase;
-  uint32_t buFound[WARPS_PER_BLOCK][32];
-  uint32_t buSlotU[WARPS_PER_BLOCK][32];
-  uint32_t buSlotTag[WARPS_PER_BLOCK][32];
-  uint32_t buList[WARPS_PER_BLOCK][BU_LIST];
+  // The two directions never run at the same time: the bottom-up lists share their memory with the slice tiles that
+  // the balanced top-down phase stages by TMA bulk copies (td_phase_b).
+  union {
+    struct {
+      uint32_t buFound[WARPS_PER_BLOCK][32];
+      uint32_t buSlotU[WARPS_PER_BLOCK][32];
+      uint32_t buSlotTag[WARPS_PER_BLOCK][32];
+      uint32_t buList[WARPS_PER_BLOCK][BU_LIST];
+    };
+    struct {
+      alignas(128) uint4 tileRows[WARPS_PER_BLOCK][2][TILE_QUADS];       // row ids of a tile: 4 slices per quad
+      alignas(16) uint32_t tileMasks[WARPS_PER_BLOCK][2][TILE_QUADS + 8];  // its masks (+ alignment slack of the copy)
+    };
+  };
+  unsigned long long tileBar[WARPS_PER_BLOCK][2];  // mbarriers of the two tile stages of every warp (never overlaid)
+  uint32_t tilePhase[WARPS_PER_BLOCK];             // their parities, kept across levels (bit s = stage s)
   uint32_t wl[WL_STAGE];
   uint32_t dcount, dvalid;      // finalisation: dense words shared by the CTA's warps
   uint2 dlist[DLIST_CAP];       // (word id, new-frontier bits)
@@ -418,16 +431,93 @@ __device__ __forceinline__ void td_phase_a(const BfsParams& p, LazyShared& sh, c
 }
 
 // Phase B: one warp per chunk, round-robin: every warp gets the same share of the hubs' bytes.
+// With options.tune[0] (ALU contraction only): the slice chunks are cut into tiles of TILE_QUADS quads and STAGED IN SHARED MEMORY BY TMA BULK COPIES
+// (cp.async.bulk + mbarrier, two stages per warp): while the warp contracts and marks tile t, the row ids and masks of
+// tile t+1 are already travelling, without occupying registers or load/store-unit slots (north_star (b); the paper's
+// profile has 39 % of Alg. 3's time waiting on these loads).  The masks of a tile start at a 4-byte
+// granularity, a bulk copy at 16 bytes: the copy starts at the aligned word below and the lanes index past the slack.
 template <int CONTR>
-__device__ __forceinline__ void td_phase_b(const BfsParams& p, uint32_t nChunks, const Marks& Fn) {
-  const uint32_t lane = threadIdx.x & 31;
-  const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
+__device__ __forceinline__ void td_phase_b(const BfsParams& p, LazyShared& sh, uint32_t nChunks, const Marks& Fn) {
+  const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + warp, nwarps = gridDim.x * WARPS_PER_BLOCK;
+  if (CONTR != 1 || !p.tmaTiles) {  // default (measured faster) and the MMA forms: 128-bit loads into registers
+    for (uint32_t i = gwarp; i < nChunks; i += nwarps) {
+      BLEST_ASSERT(i < p.chunkCap);
+      const uint4 e = __ldcg(&p.chunks[i]);
+      if (e.w) warp_edges(p, Fn, e.x, e.x + e.y, lane);
+      else warp_slices<CONTR>(p, Fn, e.x, e.y, e.z, lane);
+    }
+    return;
+  }
+  // pass 1: the edge chunks (CSR segments of hub vertices)
+  bool anySlices = false;
   for (uint32_t i = gwarp; i < nChunks; i += nwarps) {
     BLEST_ASSERT(i < p.chunkCap);
     const uint4 e = __ldcg(&p.chunks[i]);
     if (e.w) warp_edges(p, Fn, e.x, e.x + e.y, lane);
-    else warp_slices<CONTR>(p, Fn, e.x, e.y, e.z, lane);
+    else anySlices = true;
   }
+  if (!anySlices) return;
+  // pass 2: the slice chunks, tile by tile through the two-stage ring
+  uint4 (*rows)[TILE_QUADS] = sh.tileRows[warp];
+  uint32_t (*masks)[TILE_QUADS + 8] = sh.tileMasks[warp];
+  uint64_t* bar = reinterpret_cast<uint64_t*>(sh.tileBar[warp]);
+  uint32_t phase = sh.tilePhase[warp];
+  uint32_t ci = gwarp, off = 0;
+  uint4 ce = make_uint4(0, 0, 0, 1);
+  bool have = false;
+  uint32_t tStart[2], tCnt[2], tAlpha[2];
+  // next tile of this warp's slice chunks -> stage `st`; false when there is none (warp-uniform)
+  auto stage_next = [&](uint32_t st) -> bool {
+    for (;;) {
+      if (!have) {
+        if (ci >= nChunks) return false;
+        ce = __ldcg(&p.chunks[ci]);
+        have = true;
+        off = 0;
+      }
+      if (ce.w || off >= ce.y) { have = false; ci += nwarps; continue; }
+      break;
+    }
+    tStart[st] = ce.x + off;
+    tCnt[st] = min(TILE_QUADS, ce.y - off);
+    tAlpha[st] = ce.z;
+    off += TILE_QUADS;
+    if (lane == 0) {
+      const uint32_t m0 = tStart[st] & ~3u, m1 = (tStart[st] + tCnt[st] + 3u) & ~3u;
+      BLEST_ASSERT((uint64_t)tStart[st] + tCnt[st] <= p.nQuads && m1 - m0 <= TILE_QUADS + 8u);
+      mbar_arrive_expect_tx(&bar[st], tCnt[st] * 16u + (m1 - m0) * 4u);
+      bulk_g2s(rows[st], p.rowIds + tStart[st], tCnt[st] * 16u, &bar[st]);
+      bulk_g2s(masks[st], p.masks + m0, (m1 - m0) * 4u, &bar[st]);
+    }
+    return true;
+  };
+  bool live[2];
+  live[0] = stage_next(0);
+  live[1] = live[0] && stage_next(1);
+  for (uint32_t st = 0; live[st]; st ^= 1u) {
+    mbar_wait(&bar[st], (phase >> st) & 1u);
+    phase ^= 1u << st;
+    uint4 r[2];
+    uint32_t m[2];
+    const uint32_t cnt = tCnt[st], alpha = tAlpha[st], slack = tStart[st] & 3u;
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const uint32_t idx = 32u * k + lane;
+      r[k] = make_uint4(0, 0, 0, 0);
+      m[k] = 0;
+      if (idx < cnt) {
+        r[k] = rows[st][idx];
+        m[k] = masks[st][slack + idx];
+      }
+    }
+    __syncwarp();  // every lane has its quads in registers: the stage may be refilled
+    live[st] = stage_next(st);
+#pragma unroll
+    for (int k = 0; k < 2; ++k)
+      if (32u * k < cnt) mark_quad(p, Fn, r[k], contract_alu(m[k], alpha));  // (warp-uniform condition)
+  }
+  if (lane == 0) sh.tilePhase[warp] = phase;
 }
 
 // levels_out[original id of u] = level, for the set bits of up to eight words at a time (lane = bit: coalesced
@@ -896,7 +986,7 @@ __device__ __forceinline__ bool choose_bottom_up(const BfsParams& p, uint32_t le
 
 template <int CONTR>
 __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid_constant__ BfsParams p) {
-  extern __shared__ __align__(16) unsigned char lazy_smem[];
+  extern __shared__ __align__(128) unsigned char lazy_smem[];
   LazyShared& sh = *reinterpret_cast<LazyShared*>(lazy_smem);
   Ctrl* ctrl = p.ctrl;
   // The control block is never memset between calls: the barrier counter is monotone over the launches on this
@@ -908,6 +998,12 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
   const bool leader = (blockIdx.x == 0 && threadIdx.x == 0);
   if (threadIdx.x < 6) sh.acc[threadIdx.x] = 0;
   if (threadIdx.x == 0) sh.wlCnt = 0;
+  if ((threadIdx.x & 31) == 0) {  // the warp's two tile-stage barriers: one arrival (the issuing lane) + the copies' bytes
+    mbar_init(reinterpret_cast<uint64_t*>(&sh.tileBar[threadIdx.x >> 5][0]), 1u);
+    mbar_init(reinterpret_cast<uint64_t*>(&sh.tileBar[threadIdx.x >> 5][1]), 1u);
+    sh.tilePhase[threadIdx.x >> 5] = 0;
+    mbar_init_fence();
+  }
   if (leader) ctrl->t0 = globaltimer();
 
   // A4 per-call init: bitmaps cleared, V = F_curr = {src}; levels_out = -1 everywhere.
@@ -1045,7 +1141,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       const uint32_t nChunks = (uint32_t)sh.ctl[0];
       __syncthreads();
       if (nChunks) {  // hubs: equal chunks spread over the grid
-        td_phase_b<CONTR>(p, min(nChunks, p.chunkCap), mk);
+        td_phase_b<CONTR>(p, sh, min(nChunks, p.chunkCap), mk);
         grid_barrier(&ctrl->bar, epoch);
       }
       if (leader) tStage1 = globaltimer();

@@ -451,7 +451,8 @@ def test_small_graph_suite_under_bounds_asserts():
         "          lambda: gg.rmat(12, 16, 9), lambda: gg.path(2), lambda: gg.empty(1), lambda: gg.rmat(15, 16, 4)]\n"
         "opts = [dict(kernel='lazy'), dict(kernel='lazy', reorder='degree'), dict(kernel='lazy', reorder='rcm', persist_l2=False),\n"
         "        dict(kernel='lazy', switching='off'), dict(kernel='lazy', switching='bottom_up'), dict(kernel='lazy', switching='top_down'),\n"
-        "        dict(kernel='lazy', switching='slice', contraction='mma_b1'), dict(kernel='eager'), dict(kernel='eager', reorder='jaccard')]\n"
+        "        dict(kernel='lazy', switching='slice', contraction='mma_b1'), dict(kernel='eager'), dict(kernel='eager', reorder='jaccard'),\n"
+        "        dict(kernel='lazy', switching='off', tma_tiles=True, reorder='degree')]\n"
         "cases = 0\n"
         "for mk in makers:\n"
         "    n, rp, ci = mk()\n"
@@ -483,3 +484,16 @@ def test_small_graph_suite_under_bounds_asserts():
     env = dict(os.environ, BLEST_DEBUG_LIB="1", PYTHONPATH=root)
     r = subprocess.run([sys.executable, "-c", code], env=env, cwd=root, capture_output=True, text=True, timeout=900)
     assert r.returncode == 0 and "debug build ok" in r.stdout, (r.stdout[-500:], r.stderr[-2000:])
+
+
+@pytest.mark.parametrize("name", ["star_hub", "rmat12", "ragged"])
+def test_tma_staged_slice_tiles(blest, torch_cuda, name):
+    """options.tune[0]: the balanced phase of the slice path stages its tiles with cp.async.bulk + mbarrier (two stages
+    per warp, masks copied from the 16-byte-aligned word below their start).  Same levels; hub slice sets of thousands
+    of slices (star, RMAT hubs) cross many tiles and both stage parities."""
+    torch = torch_cuda
+    graph = SMALL[name]() if name != "rmat12" else gg.rmat(15, 16, 4)
+    for opts in (dict(switching="off"), dict(switching="slice", reorder="degree"), dict(switching="auto", reorder="degree")):
+        with blest.Graph(*graph, kernel="lazy", tma_tiles=True, **opts) as g:
+            check_bfs(blest, torch, g, graph, sources_for(graph[0], graph[1], 3))
+            check_bfs(blest, torch, g, graph, sources_for(graph[0], graph[1], 2))   # again: parities carried over calls
