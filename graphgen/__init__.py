@@ -78,6 +78,32 @@ def from_edges(n: int, src, dst):
     return n, rowptr, colidx[: int(nnz)]
 
 
+def from_directed_edges(n: int, src, dst):
+    """DIRECTED CSR from an edge list src -> dst: row u = sorted out-neighbours of u, loops dropped, duplicates merged.
+    (numpy; the directed test graphs are small.)"""
+    src = np.asarray(src, dtype=np.int64)
+    dst = np.asarray(dst, dtype=np.int64)
+    keep = src != dst
+    key = np.unique(src[keep] * n + dst[keep])
+    rows = key // n
+    rowptr = np.zeros(n + 1, dtype=np.int64)
+    np.add.at(rowptr, rows + 1, 1)
+    return n, np.cumsum(rowptr).astype(np.uint32), (key % n).astype(np.uint32)
+
+
+def rmat_directed(scale: int, edge_factor: int, seed: int, abc=RMAT_ABC):
+    """The RMAT draws of `rmat` kept as DIRECTED edges (not symmetrised): GAP-twitter / GAP-web are directed."""
+    L = _load()
+    n = 1 << scale
+    m = edge_factor << scale
+    src = np.empty(m, dtype=np.uint32)
+    dst = np.empty(m, dtype=np.uint32)
+    perm = np.empty(n, dtype=np.uint32)
+    L.gg_random_perm(n, seed + 2, _p(perm))
+    L.gg_rmat_edges(scale, m, seed, abc[0], abc[1], abc[2], _p(perm), _p(src), _p(dst))
+    return from_directed_edges(n, src, dst)
+
+
 def rmat(scale: int, edge_factor: int, seed: int, abc=RMAT_ABC, relabel: bool = True):
     """Graph500-style RMAT: edge_factor * 2**scale draws, then (optionally) a seeded random relabelling
     of the vertex ids so that the natural order is not accidentally degree-sorted."""

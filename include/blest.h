@@ -21,7 +21,7 @@
  *    stream-ordered allocations).  Because the calls do not wait, an error that only the device can see (an
  *    internal work-queue overflow) cannot be returned by the call that caused it: it is latched in the handle,
  *    returned by blest_last_status() and by every later traversal call on the handle until it is read there.
- *  - Graph precondition: symmetric (undirected) CSR, rows sorted ascending, column ids < n,
+ *  - Graph precondition: symmetric (undirected) CSR unless csr.directed, rows sorted ascending, column ids < n,
  *    rowptr[0] = 0, rowptr[n] = nnz < 2^32, 1 <= n <= 2^29 (narrower than uint32 because the kernels pack flags
  *    beside ids: bit 31 of a vertex id in the inline heads / bottom-up lists, 5 bits beside a slice-set id in a
  *    32-bit queue entry; the largest config has n = 2^25).  Self-loops and duplicate entries are legal and have no
@@ -52,13 +52,20 @@ enum {
                               by the kernels, reported by blest_last_status() and by later calls, never silent) */
 };
 
-/* Input graph ("CSC of A"; symmetric here, so one CSR serves as A, A^T and Alg. 4's CSR(G^T)). */
+/* Input graph ("CSC of A").  Symmetric by default, so that one CSR serves as A, A^T and Alg. 4's CSR(G^T);
+ * `directed` widens it to the paper's full problem statement. */
 typedef struct {
   uint32_t n;             /* vertices */
   uint64_t nnz;           /* directed entries = 2 * undirected edges */
   const uint32_t *rowptr; /* n+1 entries */
   const uint32_t *colidx; /* nnz entries */
   int on_device;          /* 0: host pointers, 1: device pointers (copied to the host for the host builder) */
+  int directed;           /* 0: symmetric (undirected) graph.  1: DIRECTED graph: row u lists the
+                             out-neighbours of u (the non-zeros of column u of A = the transposed adjacency matrix);
+                             levels are hop distances along the edge direction.  The library also keeps the transposed
+                             CSR (in-neighbours) for the bottom-up stage (Alg. 4 scans CSR(G^T)).
+                             Restrictions: reorder = none | degree (by out-degree); no component pruning; closeness
+                             always counts per source; blest_farness_partial is refused (BLEST_EUNSUPPORTED). */
 } blest_csr_t;
 
 /* Options.  Zero-initialised == defaults.  reorder/builder/validate are used by blest_build only; the rest

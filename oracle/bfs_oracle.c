@@ -2,8 +2,10 @@
  *
  * A plain, slow, obviously-correct implementation of what the BLEST hot path computes, written from
  * the paper, independent of the CUDA path: it shares no code, header,
- * table or helper with paper_2606_05081_b200/ and reads only the ORIGINAL symmetric uint32 CSR (no
- * BVSS, no permutation, no bitmaps).  Only tests/, __graft_entry__.smoke() and bench.py's
+ * table or helper with paper_2606_05081_b200/ and reads only the ORIGINAL uint32 CSR (no BVSS, no
+ * permutation, no bitmaps).  Row u lists the out-neighbours of u: for the symmetric configs that is
+ * simply the neighbours; for a directed graph the queue BFS follows the edge direction, which is
+ * Eq. 1 with A = the transposed adjacency matrix.  Only tests/, __graft_entry__.smoke() and bench.py's
  * cpu_baseline / --impl reference legs may call it.
  *
  * BLEST is exact, not approximate (PAPER.md:59 "The emulation is exact"; :337-339 the lazy scheme and
@@ -19,7 +21,8 @@
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): closed forms (path, cycle, grid = Manhattan,
  * complete, star, binary tree, disjoint unions, isolated source), invariants on random graphs,
  * literal Eq. 1 Boolean-matrix-power brute force for n <= 64, scipy.sparse.csgraph on larger graphs,
- * farness closed forms.  No function here is "parity unpinned".
+ * farness closed forms; the same on directed graphs (one-way path / cycle / stars, Eq. 1 with
+ * A[v][u] = 1 for u -> v, scipy directed shortest paths).  No function here is "parity unpinned".
  */
 #include <stdint.h>
 #include <stdlib.h>

@@ -36,7 +36,7 @@ class BlestError(RuntimeError):
 
 class _Csr(ctypes.Structure):
     _fields_ = [("n", ctypes.c_uint32), ("nnz", ctypes.c_uint64), ("rowptr", ctypes.c_void_p),
-                ("colidx", ctypes.c_void_p), ("on_device", ctypes.c_int)]
+                ("colidx", ctypes.c_void_p), ("on_device", ctypes.c_int), ("directed", ctypes.c_int)]
 
 
 class _Options(ctypes.Structure):
@@ -187,7 +187,7 @@ class Info:
 class Graph:
     """Owns one ``blest_handle_t``.  ``Graph(n, rowptr, colidx, reorder=..., ...)`` calls ``blest_build``."""
 
-    def __init__(self, n: int, rowptr, colidx, host_only: bool = False, **opts):
+    def __init__(self, n: int, rowptr, colidx, host_only: bool = False, directed: bool = False, **opts):
         L = load()
         self._h = ctypes.c_void_p()
         on_device = hasattr(rowptr, "data_ptr")
@@ -199,7 +199,7 @@ class Graph:
             ci = np.ascontiguousarray(colidx, dtype=np.uint32)
             nnz = int(ci.size)
         self._keep = (rp, ci)
-        csr = _Csr(int(n), nnz, _ptr(rp), _ptr(ci) if nnz else None, int(on_device))
+        csr = _Csr(int(n), nnz, _ptr(rp), _ptr(ci) if nnz else None, int(on_device), int(bool(directed)))
         self._opts = dict(opts)
         o = _options(**opts)
         fn = L.blest_preprocess_host if host_only else L.blest_build

@@ -45,6 +45,7 @@ struct blest_graph {
   blest_options_t opt{};
   blest_info_t info{};
   bool hasPerm = false;
+  bool directed = false;  // rows are out-neighbours of a directed graph; the transposed CSR is kept for Alg. 4
   bool hubby = false;     // degree-sorted AND scale-free-like: the first 1 % of the vertices own >= 20 % of the edge endpoints
   bool hostOnly = false;  // blest_preprocess_host: no device arrays, traversal calls are refused
   HostBvss hb;            // kept only when hostOnly
@@ -54,6 +55,7 @@ struct blest_graph {
   // device graph
   uint32_t *dSetPtr = nullptr, *dRowIds = nullptr, *dMasks = nullptr, *dRowptr = nullptr, *dColidx = nullptr;
   uint32_t *dPerm = nullptr, *dIperm = nullptr;
+  uint32_t *dRowptrIn = nullptr, *dColidxIn = nullptr;  // transposed CSR (== dRowptr / dColidx for a symmetric graph)
   // single-source workspace
   uint32_t nSweepWords = 0, nIsoInSweep = 0, chunkCap = 0;
   std::vector<uint32_t> setQuads;  // per slice set: quads stored          (popThr is rebuilt when gamma changes)
@@ -62,7 +64,8 @@ struct blest_graph {
   uint32_t* dDeg = nullptr;
   uint32_t* dIso = nullptr;
   uint16_t* dPopThr = nullptr;
-  std::vector<uint32_t> isoBits;  // host bitmap of zero-degree vertices (internal ids): such a source reaches nothing
+  std::vector<uint32_t> isoBits;  // host bitmap of the vertices nothing can discover (in-degree 0; internal ids)
+  std::vector<uint32_t> deadSrc;  // host bitmap of the vertices of out-degree 0: such a source reaches nothing
   std::vector<uint32_t> hubComp;  // host bitmap of the connected component of the highest-degree vertex
   uint32_t* dOutside = nullptr;   // device bitmap: NOT in that component (zero-degree vertices included)
   uint32_t nOutsideInSweep = 0;
@@ -305,8 +308,11 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
       std::memcpy(in.rowptr.data(), csr->rowptr, in.rowptr.size() * 4);
       if (csr->nnz) std::memcpy(in.colidx.data(), csr->colidx, in.colidx.size() * 4);
     }
-    rc = check_csr(in, opt.validate != 0);
+    const bool directed = csr->directed != 0;
+    if (directed && (opt.reorder == 1 || opt.reorder == 3)) return BLEST_EUNSUPPORTED;  // RCM / Jaccard: symmetric input only
+    rc = check_csr(in, opt.validate != 0 && !directed);
     if (rc) return rc;
+    g->directed = directed;
 
     // A1 reorder (timed separately, Table 7)
     double t0 = now_s();
@@ -339,13 +345,32 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
     g->nSlices = b.nSlices;
     g->nQuads = b.nQuads;
     g->nwords = (g->n + 31) / 32;
-    {  // sweep range of the lazy kernel: the 32-vertex words that hold a vertex of non-zero degree
+    // Directed graph: A = the transposed adjacency matrix, so the rows given are the COLUMNS of A (the
+    // BVSS builder reads them as such), and Alg. 4 scans IN-neighbours: the transposed CSR, by a counting sort.
+    HostCsr gin;
+    if (directed) {
+      gin.n = gcsr->n;
+      gin.nnz = gcsr->nnz;
+      gin.rowptr.assign((size_t)gin.n + 1, 0);
+      gin.colidx.resize(gin.nnz);
+      for (uint64_t e = 0; e < gcsr->nnz; ++e) ++gin.rowptr[gcsr->colidx[e] + 1];
+      for (uint32_t i = 0; i < gin.n; ++i) gin.rowptr[i + 1] += gin.rowptr[i];
+      std::vector<uint32_t> fill(gin.rowptr.begin(), gin.rowptr.end() - 1);
+      for (uint32_t u = 0; u < gcsr->n; ++u)  // ascending u: every in-list comes out sorted
+        for (uint32_t e = gcsr->rowptr[u]; e < gcsr->rowptr[u + 1]; ++e) gin.colidx[fill[gcsr->colidx[e]]++] = u;
+    }
+    const HostCsr* gcsrIn = directed ? &gin : gcsr;
+    {  // sweep range of the lazy kernel: the 32-vertex words that hold a vertex with an edge; vertices nothing can
+       // discover (in-degree 0) start out visited
       g->isoBits.assign(g->nwords, 0u);
+      g->deadSrc.assign(g->nwords, 0u);
       uint32_t last = 0;
       bool any = false;
       for (uint32_t u = 0; u < g->n; ++u) {
-        if (gcsr->rowptr[u + 1] == gcsr->rowptr[u]) g->isoBits[u >> 5] |= 1u << (u & 31u);
-        else { last = u; any = true; }
+        const bool noIn = gcsrIn->rowptr[u + 1] == gcsrIn->rowptr[u], noOut = gcsr->rowptr[u + 1] == gcsr->rowptr[u];
+        if (noIn) g->isoBits[u >> 5] |= 1u << (u & 31u);
+        if (noOut) g->deadSrc[u >> 5] |= 1u << (u & 31u);
+        if (!noIn || !noOut) { last = u; any = true; }
       }
       g->nSweepWords = any ? last / 32u + 1u : 0u;
       uint32_t iso = 0;
@@ -354,7 +379,7 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
       // Connected component of the highest-degree vertex (level-synchronous host BFS, OpenMP over the frontier).  A
       // traversal from a source inside it can never leave it, so the lazy kernel starts with everything outside marked
       // visited: no sweep ever examines those vertices, and the traversal ends as soon as the component is exhausted.
-      if (!hostOnly && any && opt.prune_components == 0) {
+      if (!hostOnly && any && opt.prune_components == 0 && !directed) {
         const double tc0 = now_s();
         uint32_t hub = 0, best = 0;
         for (uint32_t u = 0; u < g->n; ++u) {
@@ -426,6 +451,15 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
       }
       CK(cudaMemcpy(g->dRowptr, gcsr->rowptr.data(), ((size_t)g->n + 1) * 4, cudaMemcpyHostToDevice));
       if (g->nnz) CK(cudaMemcpy(g->dColidx, gcsr->colidx.data(), (size_t)g->nnz * 4, cudaMemcpyHostToDevice));
+      g->dRowptrIn = g->dRowptr;
+      g->dColidxIn = g->dColidx;
+      if (directed) {
+        if ((rc = dev_alloc(g, &g->dRowptrIn, (uint64_t)g->n + 1))) return rc;
+        if ((rc = dev_alloc(g, &g->dColidxIn, g->nnz))) return rc;
+        g->info.csr_bytes += ((uint64_t)g->n + 1 + g->nnz) * 4;
+        CK(cudaMemcpy(g->dRowptrIn, gin.rowptr.data(), ((size_t)g->n + 1) * 4, cudaMemcpyHostToDevice));
+        if (g->nnz) CK(cudaMemcpy(g->dColidxIn, gin.colidx.data(), (size_t)g->nnz * 4, cudaMemcpyHostToDevice));
+      }
       if (g->hasPerm) {
         if ((rc = dev_alloc(g, &g->dPerm, g->n))) return rc;
         if ((rc = dev_alloc(g, &g->dIperm, g->n))) return rc;
@@ -438,12 +472,12 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
         std::vector<uint32_t> deg(g->n);
 #pragma omp parallel for schedule(static)
         for (int64_t u = 0; u < (int64_t)g->n; ++u) {
-          const uint32_t b0 = gcsr->rowptr[u], d = gcsr->rowptr[u + 1] - b0;
+          const uint32_t b0 = gcsrIn->rowptr[u], d = gcsrIn->rowptr[u + 1] - b0;  // in-neighbours (Alg. 4)
           uint2 hd = make_uint2(0xFFFFFFFFu, 0xFFFFFFFFu);
-          if (d >= 1) hd.x = gcsr->colidx[b0];
-          if (d >= 2) hd.y = gcsr->colidx[b0 + 1] | (d > 2 ? 0x80000000u : 0u);
+          if (d >= 1) hd.x = gcsrIn->colidx[b0];
+          if (d >= 2) hd.y = gcsrIn->colidx[b0 + 1] | (d > 2 ? 0x80000000u : 0u);
           head[u] = hd;
-          deg[u] = d;
+          deg[u] = gcsr->rowptr[u + 1] - gcsr->rowptr[u];  // out-degree: what a frontier vertex expands
         }
         g->setQuads.resize(g->Ns);
         g->setDeg.resize(g->Ns);
@@ -603,6 +637,7 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
   p.nQuads = h->nQuads; p.wlCap = h->nSweepWords + 16384u;
   p.setPtr = h->dSetPtr; p.rowIds = reinterpret_cast<const uint4*>(h->dRowIds); p.masks = h->dMasks;
   p.rowptr = h->dRowptr; p.colidx = h->dColidx;
+  p.rowptrIn = h->dRowptrIn; p.colidxIn = h->dColidxIn;
   p.perm = h->hasPerm ? h->dPerm : nullptr;
   p.iperm = h->hasPerm ? h->dIperm : nullptr;
   p.nSweepWords = h->nSweepWords; p.nIsoInSweep = h->nIsoInSweep; p.isoBits = h->dIso;
@@ -641,7 +676,8 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
   p.tmaTiles = h->opt.tune[0] == 1;
   p.eta = h->opt.eta;
   p.gamma = h->opt.gamma;
-  if ((h->isoBits[p.src >> 5] >> (p.src & 31u)) & 1u) {
+  p.srcPremarked = (p.isoBits == h->dIso) ? (int)((h->isoBits[p.src >> 5] >> (p.src & 31u)) & 1u) : 0;
+  if ((h->deadSrc[p.src >> 5] >> (p.src & 31u)) & 1u) {
     h->lastCtrl = nullptr;
     CK(launch_isolated_source(p.out, h->n, src, st));  // nothing to traverse
   } else if (resolved_kernel(h) == 1) {
@@ -853,11 +889,13 @@ static int closeness_impl(blest_handle_t h, const uint32_t* srcs, uint64_t n_src
   MsParams p{};
   fill_ms_params(h, p);
   p.nsrcs = n_srcs;
-  if (srcs) {  // arbitrary subset: per-source counts (reading R13)
-    e = tmp.alloc((void**)&dSrcs, n_srcs * 4);
+  if (srcs || h->directed) {
+    // arbitrary subset: per-source counts (reading R13).  Also every run on a DIRECTED graph: the target-side sums of
+    // Eq. 7 are the farness of the reached vertex only when d(s, u) = d(u, s).
+    if (srcs) e = tmp.alloc((void**)&dSrcs, n_srcs * 4);
     if (e == cudaSuccess) e = tmp.alloc((void**)&dFarS, n_srcs * 8);
     if (e == cudaSuccess) e = tmp.alloc((void**)&dReachS, n_srcs * 4);
-    if (e == cudaSuccess) e = stage_srcs(h, srcs, n_srcs, dSrcs, st);
+    if (e == cudaSuccess && srcs) e = stage_srcs(h, srcs, n_srcs, dSrcs, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(dFarS, 0, n_srcs * 8, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(dReachS, 0, n_srcs * 4, st);
     p.srcs = dSrcs;
@@ -894,6 +932,7 @@ int blest_farness_partial(blest_handle_t h, uint32_t first, uint32_t count, uint
   if (!h || !far_sum || !reach_sum || count == 0) return BLEST_EINVAL;
   if (h->hostOnly) return BLEST_EUNSUPPORTED;
   if ((uint64_t)first + count > h->n) return BLEST_EINVAL;
+  if (h->directed) return BLEST_EUNSUPPORTED;  // target-side sums need d(s, u) = d(u, s)
   if (!is_device_ptr(far_sum) || !is_device_ptr(reach_sum)) return BLEST_EINVAL;
   if (int rc = pending_status(h)) return rc;
   cudaStream_t st = (cudaStream_t)cuda_stream;

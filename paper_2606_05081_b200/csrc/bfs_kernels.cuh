@@ -20,12 +20,15 @@ struct BfsParams {
   const uint32_t* setPtr;  // Ns+1 quad offsets
   const uint4* rowIds;     // nQuads
   const uint32_t* masks;   // nQuads
-  const uint32_t* rowptr;  // internal (reordered) CSR, n+1
+  const uint32_t* rowptr;  // internal (reordered) CSR, n+1: OUT-neighbours (the columns of A; top-down edge path)
   const uint32_t* colidx;
+  const uint32_t* rowptrIn;  // CSR of the transposed graph: IN-neighbours (Alg. 4's CSR(G^T)); the same
+  const uint32_t* colidxIn;  // arrays as rowptr / colidx when the graph is symmetric
+  int srcPremarked;          // the source's bit is already set in isoBits (directed graph, source of in-degree 0)
   const uint32_t* perm;    // original -> internal id, or nullptr when no reordering
   const uint32_t* iperm;   // internal -> original id, or nullptr when no reordering
-  const uint2* head;       // n: first two neighbours of every vertex (x, y); 0xFFFFFFFF = none; y bit 31 = "has more"
-  const uint32_t* deg;     // n: degrees (read where a discovered vertex is finalised, for the switch counters)
+  const uint2* head;       // n: first two IN-neighbours of every vertex (x, y); 0xFFFFFFFF = none; y bit 31 = "has more"
+  const uint32_t* deg;     // n: OUT-degrees (read where a discovered vertex is finalised, for the switch counters)
   const uint16_t* popThr;  // nwords: four 4-bit thresholds, one per slice set of the word (slice path iff
                            // popc(frontier byte) >= threshold; 9 = never)
   // lazy kernel state

@@ -744,7 +744,7 @@ __device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_
       if ((more >> k) & 1u) {
         BLEST_ASSERT(listCount + pos[k] < BU_LIST);
         list[listCount + pos[k]] = u[k] | CSR_STAGE;
-        prefetch_l2(&p.rowptr[u[k]]);
+        prefetch_l2(&p.rowptrIn[u[k]]);
       }
     listCount += total;
     __syncwarp();
@@ -765,8 +765,8 @@ __device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_
     if (mine) {
       const uint32_t uu = slotU[lane] & ~CSR_STAGE;
       tag = slotTag[lane];
-      ptr = __ldg(&p.rowptr[uu]) + 2u;
-      e = __ldg(&p.rowptr[uu + 1]);
+      ptr = __ldg(&p.rowptrIn[uu]) + 2u;
+      e = __ldg(&p.rowptrIn[uu + 1]);
       c.qbytes += 8ull;
     }
     bool f = false;
@@ -776,7 +776,7 @@ __device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_
       const uint32_t cnt = min(4u, stop - ptr);
       BLEST_ASSERT((uint64_t)ptr + cnt <= p.nnz);
 #pragma unroll
-      for (int j = 0; j < 4; ++j) v[j] = (uint32_t)j < cnt ? __ldg(&p.colidx[ptr + j]) : 0u;
+      for (int j = 0; j < 4; ++j) v[j] = (uint32_t)j < cnt ? __ldg(&p.colidxIn[ptr + j]) : 0u;
 #pragma unroll
       for (int j = 0; j < 4; ++j) fwd[j] = (uint32_t)j < cnt ? Fp[v[j] >> 5] : 0u;
 #pragma unroll
@@ -797,7 +797,7 @@ __device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_
         const uint32_t idx = b2 + lane;
         bool hit = false;
         if (idx < E) {
-          const uint32_t v = __ldg(&p.colidx[idx]);
+          const uint32_t v = __ldg(&p.colidxIn[idx]);
           hit = (Fp[v >> 5] >> (v & 31u)) & 1u;
           ++c.scanned;
           c.qbytes += 4ull;
@@ -1043,7 +1043,8 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     ctrl->wlc[0] = 1;
     ctrl->newcount[0] = 1;
     ctrl->mf[0] = srcDeg;
-    ctrl->unvisited[0] = (unsigned long long)min((uint64_t)p.n, (uint64_t)nSW * 32u) - 1u - p.nIsoInSweep;
+    // (the source is not counted twice when it is itself pre-marked: a directed graph's source of in-degree 0)
+    ctrl->unvisited[0] = (unsigned long long)min((uint64_t)p.n, (uint64_t)nSW * 32u) - (p.srcPremarked ? 0u : 1u) - p.nIsoInSweep;
   }
   grid_barrier(&ctrl->bar, epoch);
   if (leader) {

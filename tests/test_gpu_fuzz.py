@@ -43,7 +43,11 @@ def test_fuzz_single_source():
         reorder = ["none", "degree", "rcm", "jaccard"][int(rng.integers(0, 4))]
         kernel = ["auto", "lazy", "lazy", "eager"][int(rng.integers(0, 4))]
         switching = ["auto", "auto", "auto", "off", "bottom_up", "top_down", "slice"][int(rng.integers(0, 7))]
-        with blest.Graph(n, rp, ci, reorder=reorder, kernel=kernel, switching=switching) as g:
+        directed = cases % 5 == 4
+        if directed:  # every fifth case: a directed graph with the same vertex count and about as many edges
+            n, rp, ci = gg.from_directed_edges(n, rng.integers(0, n, max(ci.size // 2, 1)), rng.integers(0, n, max(ci.size // 2, 1)))
+            reorder = reorder if reorder in ("none", "degree") else "degree"
+        with blest.Graph(n, rp, ci, reorder=reorder, kernel=kernel, switching=switching, directed=directed) as g:
             out = torch.full((n,), 7, dtype=torch.int32, device="cuda")
             for s in sorted(set([0, n - 1] + [int(x) for x in rng.integers(0, n, size=2)])):
                 g.bfs(s, out)

@@ -497,3 +497,62 @@ def test_tma_staged_slice_tiles(blest, torch_cuda, name):
         with blest.Graph(*graph, kernel="lazy", tma_tiles=True, **opts) as g:
             check_bfs(blest, torch, g, graph, sources_for(graph[0], graph[1], 3))
             check_bfs(blest, torch, g, graph, sources_for(graph[0], graph[1], 2))   # again: parities carried over calls
+
+
+# ---- directed graphs (NEXT 4) -------------------------------------------------------------------
+def directed_graphs():
+    rng = np.random.Generator(np.random.PCG64(38))
+    n = 3001
+    yield "gnm", gg.from_directed_edges(n, rng.integers(0, n, 9000), rng.integers(0, n, 9000))
+    yield "rmat13", gg.rmat_directed(13, 8, 7)
+    i = np.arange(999)
+    yield "path", gg.from_directed_edges(1000, i, i + 1)                              # 999 levels one way, nothing back
+    yield "instar", gg.from_directed_edges(4000, np.arange(1, 4000), np.zeros(3999, int))   # hub of in-degree 3999
+    yield "outstar", gg.from_directed_edges(4000, np.zeros(3999, int), np.arange(1, 4000))  # hub slice set, leaves are dead ends
+    yield "dag", gg.from_directed_edges(600, rng.integers(0, 300, 2000), rng.integers(300, 600, 2000))  # sources with in-degree 0
+
+
+@pytest.mark.parametrize("name", ["gnm", "rmat13", "path", "instar", "outstar", "dag"])
+def test_directed_graphs_every_path(blest, torch_cuda, name):
+    """Levels along the edge direction, bit-exact against the oracle, through every kernel and forced path: top-down reads
+    the out-neighbour CSR / the BVSS of A, bottom-up (Alg. 4) the transposed CSR the library builds."""
+    torch = torch_cuda
+    graph = dict(directed_graphs())[name]
+    n, rp, ci = graph
+    indeg = np.bincount(ci, minlength=n)
+    srcs = sorted({0, n - 1, int(np.argmax(np.diff(rp.astype(np.int64)))), int(np.argmax(indeg)), int(np.argmin(indeg))})
+    for opts in (dict(kernel="lazy"), dict(kernel="lazy", reorder="degree"), dict(kernel="lazy", reorder="degree", persist_l2=False),
+                 dict(kernel="lazy", switching="off"), dict(kernel="lazy", switching="bottom_up"),
+                 dict(kernel="lazy", switching="top_down"), dict(kernel="lazy", switching="scripted", bu_mask=0b10101010),
+                 dict(kernel="eager"), dict(kernel="eager", reorder="degree")):
+        with blest.Graph(n, rp, ci, directed=True, **opts) as g:
+            check_bfs(blest, torch, g, graph, srcs)
+            assert g.last_status() == 0
+
+
+@pytest.mark.parametrize("kappa", [32, 64, 256])
+def test_directed_msbfs_and_closeness(blest, torch_cuda, kappa):
+    """Multi-source rows = single-source levels; closeness of all vertices on a directed graph counts per source (the
+    target-side sums of Eq. 7 would be the IN-farness): bit-equal to the oracle; the partial-sum call is refused."""
+    from paper_2606_05081_b200 import binding
+
+    torch = torch_cuda
+    n, rp, ci = gg.rmat_directed(10, 8, 3)
+    far_w, reach_w, cc_w, _ = oracle.closeness(n, rp, ci)
+    for reorder in ("none", "degree"):
+        with blest.Graph(n, rp, ci, directed=True, kappa=kappa, reorder=reorder) as g:
+            srcs = np.array([0, 5, 5, n - 1, 77] + list(range(100, 100 + kappa)), dtype=np.uint32)
+            lv = torch.empty((srcs.size, n), dtype=torch.int32, device="cuda")
+            g.msbfs(srcs, lv)
+            assert np.array_equal(lv.cpu().numpy(), oracle.msbfs(n, rp, ci, srcs))
+            far = torch.zeros(n, dtype=torch.int64, device="cuda")
+            reach = torch.zeros(n, dtype=torch.int32, device="cuda")
+            g.farness(far, reach)
+            assert np.array_equal(far.cpu().numpy().view(np.uint64), far_w)
+            assert np.array_equal(reach.cpu().numpy().view(np.uint32), reach_w)
+            cc = torch.zeros(n, dtype=torch.float64, device="cuda")
+            g.closeness(cc)
+            assert np.array_equal(cc.cpu().numpy(), cc_w)
+            with pytest.raises(blest.BlestError) as e:
+                g.farness_partial(0, 64, far, reach)
+            assert e.value.status == binding.EUNSUPPORTED

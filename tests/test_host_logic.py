@@ -223,3 +223,24 @@ def test_jaccard_with_windows_groups_overlapping_columns():
     d_deg = blest.Graph(n2, rp2, ci2, host_only=True, reorder="degree").info().mask_density
     d_jac = blest.Graph(n2, rp2, ci2, host_only=True, reorder="jaccard").info().mask_density
     assert d_jac >= d_deg
+
+
+@pytest.mark.parametrize("reorder", ["none", "degree"])
+def test_bvss_of_a_directed_graph(reorder):
+    """A is the TRANSPOSED adjacency matrix, so an edge u -> v is the non-zero A[v][u]: the slice of row v in
+    the slice set of column u.  Decoding the BVSS of a directed CSR must give exactly the edges, as (row = head,
+    column = tail) pairs; RCM / Jaccard need a symmetric input and are refused."""
+    n, rp, ci = gg.rmat_directed(10, 8, 5)
+    g = blest.Graph(n, rp, ci, host_only=True, directed=True, reorder=reorder)
+    irp, ici = g.array("rowptr").astype(np.int64), g.array("colidx").astype(np.int64)
+    perm = g.array("perm").astype(np.int64) if reorder != "none" else np.arange(n)
+    tails_o = np.repeat(np.arange(n), np.diff(rp.astype(np.int64)))
+    tails_i = np.repeat(np.arange(n), np.diff(irp))
+    assert np.array_equal(np.sort(perm[tails_o] * n + perm[ci.astype(np.int64)]), tails_i * n + ici)   # same directed edges
+    r, c, mb, rowIds, setPtr, set_of_slice = decode_bvss(g)
+    assert np.array_equal(np.sort(c * n + r), tails_i * n + ici)          # column = tail u, row = head v
+    assert not np.array_equal(np.sort(r * n + c), tails_i * n + ici)      # (and not the other way round: the graph is asymmetric)
+    assert int(np.unpackbits(mb).sum()) == ci.size
+    for bad in ("rcm", "jaccard"):
+        with pytest.raises(blest.BlestError):
+            blest.Graph(n, rp, ci, host_only=True, directed=True, reorder=bad)

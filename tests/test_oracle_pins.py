@@ -189,3 +189,75 @@ def test_component_edges():
     g = gg.disjoint_union(gg.path(4), gg.complete(5))
     assert oracle.component_edges(g[1], oracle.bfs(*g, 0)) == 3
     assert oracle.component_edges(g[1], oracle.bfs(*g, 6)) == 10
+
+
+# ---- directed graphs (A is the TRANSPOSED adjacency matrix; BFS follows the edge direction) ----------
+def eq1_levels_directed(n, rowptr, colidx, src):
+    """Eq. 1 literally, on a DIRECTED CSR whose row u lists the out-neighbours of u: edge u -> v is A[v][u] = 1."""
+    rows = [0] * n
+    for u in range(n):
+        for e in range(int(rowptr[u]), int(rowptr[u + 1])):
+            rows[int(colidx[e])] |= 1 << u
+    x = v = 1 << src
+    level = [-1] * n
+    level[src] = 0
+    k = 0
+    while x:
+        nxt = 0
+        for i in range(n):
+            if (rows[i] & x) != 0 and not (v >> i) & 1:
+                nxt |= 1 << i
+        k += 1
+        for i in range(n):
+            if (nxt >> i) & 1:
+                level[i] = k
+        v |= nxt
+        x = nxt
+    return np.array(level, dtype=np.int32)
+
+
+def test_directed_closed_forms():
+    n = 17
+    i = np.arange(n - 1)
+    dpath = gg.from_directed_edges(n, i, i + 1)                      # 0 -> 1 -> ... -> n-1
+    for s in (0, 5, n - 1):
+        want = np.where(np.arange(n) >= s, np.arange(n) - s, -1)     # only forward vertices are reachable
+        assert np.array_equal(oracle.bfs(*dpath, s), want)
+    dcycle = gg.from_directed_edges(n, np.arange(n), (np.arange(n) + 1) % n)
+    for s in (0, 9):
+        assert np.array_equal(oracle.bfs(*dcycle, s), (np.arange(n) - s) % n)   # one way round, not min of both
+    out_star = gg.from_directed_edges(n, np.zeros(n - 1, int), np.arange(1, n))
+    assert np.array_equal(oracle.bfs(*out_star, 0), [0] + [1] * (n - 1))
+    assert np.array_equal(oracle.bfs(*out_star, 3), [-1] * 3 + [0] + [-1] * (n - 4))     # a leaf reaches nothing
+    in_star = gg.from_directed_edges(n, np.arange(1, n), np.zeros(n - 1, int))
+    assert np.array_equal(oracle.bfs(*in_star, 3), [1] + [-1] * 2 + [0] + [-1] * (n - 4))
+    far, reach, cc, _ = oracle.closeness(*dpath, np.array([0, n - 1], np.uint32))
+    assert list(far) == [n * (n - 1) // 2, 0] and list(reach) == [n, 1] and cc[1] == 0.0
+
+
+@pytest.mark.parametrize("n,m,seed", [(2, 1, 1), (13, 20, 3), (31, 60, 4), (64, 100, 5), (64, 600, 6), (64, 4000, 7), (40, 30, 8)])
+def test_directed_bruteforce_eq1(n, m, seed):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    g = gg.from_directed_edges(n, rng.integers(0, n, m), rng.integers(0, n, m))
+    for s in sorted({0, n // 2, n - 1}):
+        assert np.array_equal(oracle.bfs(*g, s), eq1_levels_directed(*g, s))
+
+
+def test_directed_against_scipy_and_invariants():
+    import scipy.sparse as sp
+    from scipy.sparse.csgraph import shortest_path
+
+    n, rp, ci = gg.rmat_directed(12, 8, 21)
+    A = sp.csr_matrix((np.ones(ci.size), ci.astype(np.int64), rp.astype(np.int64)), shape=(n, n))
+    srcs = [0, 17, n - 1, int(np.argmax(np.diff(rp.astype(np.int64))))]
+    d = shortest_path(A, method="D", directed=True, unweighted=True, indices=srcs)
+    rows = np.repeat(np.arange(n), np.diff(rp.astype(np.int64)))
+    for k, s in enumerate(srcs):
+        lv = oracle.bfs(n, rp, ci, s)
+        assert np.array_equal(lv, np.where(np.isinf(d[k]), -1, d[k]).astype(np.int32))
+        lu, lw = lv[rows].astype(np.int64), lv[ci].astype(np.int64)
+        ok = lu >= 0
+        assert np.all(lw[ok] >= 0) and np.all(lw[ok] <= lu[ok] + 1)      # u -> w: w is reached, at most one level later
+        has_parent = np.zeros(n, bool)
+        has_parent[ci[ok & (lw == lu + 1)]] = True
+        assert np.all(has_parent[lv > 0])                                # every vertex at L > 0 has an in-neighbour at L-1
