@@ -503,6 +503,8 @@ def main():
     ap.add_argument("--contraction", default="auto")
     ap.add_argument("--reorder", default=None)
     ap.add_argument("--kappa", type=int, default=64)
+    ap.add_argument("--tma-tiles", action="store_true", help="options.tune[0]: TMA-staged slice tiles in the balanced phase")
+    ap.add_argument("--keep-trace", action="store_true", help="leave the per-level trace on inside the timed region")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     want_cpu = not (args.no_cpu_baseline or args.no_parity)
@@ -557,7 +559,8 @@ def main():
     reorder = args.reorder or REORDER_FOR[args.config]
     log(f"[rank {rank}] {args.config} shrink {args.shrink}: n={n} nnz={ci.size} gen {gen_s:.1f}s; building (reorder={reorder})")
     t0 = time.perf_counter()
-    g = blest.Graph(n, rp, ci, reorder=reorder, kernel=args.kernel, switching=args.switching, contraction=args.contraction)
+    g = blest.Graph(n, rp, ci, reorder=reorder, kernel=args.kernel, switching=args.switching, contraction=args.contraction,
+                    tma_tiles=args.tma_tiles)
     build_wall = time.perf_counter() - t0
     info = g.info()
     stream = torch.cuda.Stream()
@@ -601,6 +604,9 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    # the per-level trace is a diagnostic (its records fed the byte counts above): the timed calls run without it
+    if not args.keep_trace:
+        g.configure(trace=False)
     for _ in range(args.warmup):
         one_step(out)
     barrier()
@@ -656,6 +662,7 @@ def main():
     barrier()
     e2e_ov_ms = e0.elapsed_time(e1)
     clocks = sampler.stop() if sampler else None
+    g.configure(trace=True)
 
     # oracle legs (rank 0): cpu_baseline + parity + TEPS numerators from the oracle's levels
     base, parity, edges = None, None, gpu_edges

@@ -83,7 +83,8 @@ typedef struct {
   int contraction; /* 0 auto | 1 ALU (AND + per-byte test) | 2 mma.sync m8n8k128 b1 and.popc (paper layout, Fig. 3) |
                       3 mma.sync m16n8k32 u8 (bits expanded to bytes) */
   int kappa;       /* multi-source width: 0 -> 64 | 32 | 64 | 128 | 256 (reading R19) */
-  int trace;       /* 0 | 1: keep the per-level trace (always cheap; default on) */
+  int trace;       /* 0 | 1: keep the per-level trace / the multi-source totals of the last call (default) | 2: off (the
+                      leader thread then writes no record after a level: about a microsecond per level) */
   float eta;       /* bottom-up switch constant (Eq. 6, eta = 10 on Hopper); 0 -> library default */
   float gamma;     /* scales the slice-path cost in the per-slice-set slice-vs-CSR-edges threshold; 0 -> 1.0 */
   int persist_l2;  /* 0 auto | 1 off.  auto: a single-source traversal of a REORDERED graph whose 4n-byte levels_out

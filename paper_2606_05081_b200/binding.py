@@ -162,7 +162,7 @@ def _options(reorder="none", builder=0, validate=False, kernel="auto", switching
     o.switching = SWITCHING[switching] if isinstance(switching, str) else int(switching)
     o.contraction = CONTRACTION[contraction] if isinstance(contraction, str) else int(contraction)
     o.kappa = int(kappa)
-    o.trace = int(bool(trace))
+    o.trace = 1 if trace else 2
     o.eta = float(eta)
     o.gamma = float(gamma)
     o.persist_l2 = 0 if persist_l2 else 1

@@ -657,7 +657,7 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
   p.L = h->hasPerm ? h->dL : p.out;
   p.stamp = h->dStamp;
   p.hostStatus = h->hStatus;
-  p.trace = h->opt.trace == 0 || h->opt.trace == 1 ? h->dTrace : nullptr;
+  p.trace = h->opt.trace != 2 ? h->dTrace : nullptr;
   p.traceCap = TRACE_CAP;
   p.src = h->hasPerm ? h->perm[src] : src;
   p.srcOrig = src;
@@ -778,7 +778,7 @@ static void fill_ms_params(blest_graph* h, MsParams& p) {
   p.ctrl = h->dCtrl;
   p.hostStatus = h->hStatus;
   p.kappa = h->opt.kappa;
-  p.stats = h->opt.trace ? h->dMsStats : nullptr;
+  p.stats = h->opt.trace != 2 ? h->dMsStats : nullptr;
 }
 
 // Stream-ordered temporaries of one multi-source call: device buffers from the stream's memory pool
