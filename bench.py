@@ -504,6 +504,7 @@ def main():
     ap.add_argument("--reorder", default=None)
     ap.add_argument("--kappa", type=int, default=64)
     ap.add_argument("--tma-tiles", action="store_true", help="options.tune[0]: TMA-staged slice tiles in the balanced phase")
+    ap.add_argument("--no-persist", action="store_true", help="options.persist_l2 = off: internal-id levels + gather hand-off")
     ap.add_argument("--keep-trace", action="store_true", help="leave the per-level trace on inside the timed region")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
@@ -560,7 +561,7 @@ def main():
     log(f"[rank {rank}] {args.config} shrink {args.shrink}: n={n} nnz={ci.size} gen {gen_s:.1f}s; building (reorder={reorder})")
     t0 = time.perf_counter()
     g = blest.Graph(n, rp, ci, reorder=reorder, kernel=args.kernel, switching=args.switching, contraction=args.contraction,
-                    tma_tiles=args.tma_tiles)
+                    tma_tiles=args.tma_tiles, persist_l2=not args.no_persist)
     build_wall = time.perf_counter() - t0
     info = g.info()
     stream = torch.cuda.Stream()
@@ -696,6 +697,7 @@ def main():
                 "sources_per_step": int(len(srcs)), "l2": "inputs larger than L2 (BVSS+CSR >> 126 MB)" if info.bvss_bytes > (1 << 28) else "L2-resident graph (no flush: the paper's workload re-traverses a resident graph)",
                 "kernel": {1: "eager (Alg. 2)", 2: "lazy (Alg. 3) + switching"}[info.kernel_chosen],
                 "parallelism": "replicas only (own sources per rank)" if world > 1 else "1 GPU",
+                "hand_off": "gather pass (persist_l2 off)" if args.no_persist else "fused scatter under a persisting-L2 window when levels_out fits it",
                 "teps_numerator": "oracle levels" if parity else "GPU levels (oracle legs skipped)",
                 "bvss_bytes": int(info.bvss_bytes), "csr_bytes": int(info.csr_bytes), "mask_density": info.mask_density, "u_div": info.u_div,
                 "gen_seconds": gen_s, "reorder_seconds": info.reorder_seconds, "bvss_build_seconds": info.build_seconds,
