@@ -43,6 +43,7 @@ struct LazyShared {
   unsigned long long ctl[4];  // control words of the level, read by one thread and broadcast
   uint32_t wlCnt;
   uint32_t wlBase;
+  uint32_t buDecision;  // direction of the level, evaluated by the thread that read the control words
   // The two directions never run at the same time: the bottom-up lists share their memory with the slice tiles that
   // the balanced top-down phase stages by TMA bulk copies (td_phase_b).
   union {
@@ -1062,19 +1063,21 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       sh.ctl[1] = ld_volatile(&ctrl->mf[cp]);
       sh.ctl[2] = ld_volatile(&ctrl->unvisited[cp]);
       sh.ctl[3] = ld_volatile(&ctrl->wlc[cp]);
+      // the switch (a powf and an expf) is evaluated once per CTA, not by every warp
+      const unsigned long long dv = degVisited + sh.ctl[1];
+      sh.buDecision = choose_bottom_up(p, level, sh.ctl[0], sh.ctl[1], sh.ctl[2], p.nnz > dv ? p.nnz - dv : 0ull) ? 1u : 0u;
     }
     __syncthreads();
     const unsigned long long nf = sh.ctl[0];
     const unsigned long long mf = sh.ctl[1];
     const unsigned long long unvAll = sh.ctl[2];
     const uint32_t wlCount = (uint32_t)sh.ctl[3];
+    const bool bottomUp = sh.buDecision != 0u;
     __syncthreads();
     if (nf == 0) break;  // empty frontier ("terminates at the first level with x = 0")
     if (unvAll == 0) break;  // nothing left that could be discovered (everything outside the component is pre-marked)
     degVisited += mf;
     const unsigned long long nu = unvAll;  // zero-degree vertices count as visited from the start
-    const unsigned long long mu = p.nnz > degVisited ? p.nnz - degVisited : 0ull;
-    const bool bottomUp = choose_bottom_up(p, level, nf, mf, nu, mu);
     const uint32_t* Fp = p.F[cp];
     uint32_t* Fn = p.F[ci];
     uint32_t* Fs = p.F[cn];
