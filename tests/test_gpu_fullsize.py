@@ -159,3 +159,25 @@ def test_full_size_c5_closeness_sampled(env, kappa):
     lv = oracle.bfs(n, rp, ci, int(sample[np.argmax(reach_w)]))
     comp = lv >= 0
     assert np.all(reach_g[comp] == reach_g[comp][0])
+
+
+def test_large_directed_rmat(env):
+    """A directed graph at a size where every phase of the lazy kernel runs (RMAT scale 21, 16 M directed edges, hub
+    slice sets, bottom-up levels over the transposed CSR, degree order): levels of four sources element by element,
+    default switch and forced bottom-up."""
+    torch, blest = env
+    n, rp, ci = gg.rmat_directed(21, 8, 4711)
+    outdeg = np.diff(rp.astype(np.int64))
+    indeg = np.bincount(ci, minlength=n)
+    srcs = [int(np.argmax(outdeg)), int(np.flatnonzero((outdeg > 0) & (indeg == 0))[0]), int(np.flatnonzero(outdeg > 3)[1000]),
+            int(np.flatnonzero(outdeg == 0)[0])]
+    want = [oracle.bfs(n, rp, ci, s) for s in srcs]
+    assert max(int(w.max()) for w in want) >= 4 and min(int((w >= 0).sum()) for w in want) == 1   # deep traversals and a dead end
+    out = torch.empty(n, dtype=torch.int32, device="cuda")
+    for opts in (dict(reorder="degree"), dict(reorder="none", switching="bottom_up"), dict(reorder="degree", kernel="eager")):
+        with blest.Graph(n, rp, ci, directed=True, **opts) as g:
+            for s, w in zip(srcs, want):
+                g.bfs(s, out)
+                got = out.cpu().numpy()
+                assert np.array_equal(got, w), (opts, s, int(np.count_nonzero(got != w)))
+            assert g.last_status() == 0
