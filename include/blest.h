@@ -184,6 +184,22 @@ int blest_farness_partial(blest_handle_t h, uint32_t first, uint32_t count, uint
 int blest_closeness_from_sums(const uint64_t *far_sum, const uint32_t *reach_sum, uint64_t n, double *out,
                               void *cuda_stream);
 
+/* Allocation-free closeness of a source subset, for callers that cannot allocate (CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc).  Same result as blest_closeness(h, srcs, n_srcs, out, stream) (Eq. 7-8 with
+ * per-source counts, reading R13), but the call performs NO cudaMalloc / cudaFree / cudaMallocAsync / cudaHostAlloc:
+ * its scratch (the kappa-bit state arrays, dirtySets, the per-source sums, a copy of the source ids) lives in ONE
+ * file-scope `static __device__` array of about 6.2 MiB that every GPU loading the library holds until the process
+ * exits; the work queues and the control block are the handle's (allocated by blest_build).
+ *   srcs_dev  DEVICE uint32[n_srcs], original ids (ids >= n are a caller error; they are clamped to n - 1, not checked);
+ *   out_dev   DEVICE double[n_srcs].
+ * Limits (BLEST_ERANGE beyond them, nothing is truncated; see blest_noalloc_limits): n_srcs <= 4096;
+ * ceil(n/8) * 8 * kappa/8 <= 2 MiB, i.e. n <= 262 144 at kappa = 64, 65 536 at kappa = 256; n <= 524 288.
+ * The array is shared by ALL calls and handles of the process and keeps the last call's contents; what must start at
+ * zero is cleared at the start of each call on `cuda_stream`.  Calls that overlap on the GPU (different streams without
+ * ordering) race on it: keep them stream-ordered. */
+int blest_closeness_noalloc(blest_handle_t h, const uint32_t *srcs_dev, uint32_t n_srcs, double *out_dev, void *cuda_stream);
+int blest_noalloc_limits(uint32_t *max_srcs, uint64_t *max_state_bytes, uint64_t *max_vertices_at_kappa64);
+
 /* Totals of the most recent multi-source launch, for the roofline (needs options.trace): out8[0] work-queue entries
  * (VSS chunks) consumed by Stage 1, [1] quads they hold, [2] slices whose V_next word was probed, [3] row words updated
  * by an atomic, [4] dirty slice sets swept by Stage 2, [5] levels, [6] source batches, [7] 0.  Synchronises the device. */

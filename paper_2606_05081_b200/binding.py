@@ -71,7 +71,7 @@ TRACE_DTYPE = np.dtype([("level", "<u4"), ("mode", "<u4"), ("q_entries", "<u4"),
 
 EXPORTS = ["blest_build", "blest_preprocess_host", "blest_configure", "blest_get_call_stats", "blest_bfs", "blest_msbfs", "blest_closeness", "blest_farness",
            "blest_get_info", "blest_last_status", "blest_farness_partial", "blest_closeness_from_sums", "blest_get_ms_stats",
-           "blest_l2_microbench", "blest_tcgen05_microbench", "blest_get_trace", "blest_get_array", "blest_get_vi", "blest_contraction_selftest",
+           "blest_l2_microbench", "blest_tcgen05_microbench", "blest_closeness_noalloc", "blest_noalloc_limits", "blest_get_trace", "blest_get_array", "blest_get_vi", "blest_contraction_selftest",
            "blest_mma_microbench", "blest_barrier_microbench", "blest_destroy", "blest_strerror",
            "blest_last_cuda_error"]
 
@@ -102,6 +102,8 @@ def load(build_if_missing: bool = True):
     L.blest_farness_partial.argtypes = [vp, u32, u32, vp, vp, vp]
     L.blest_closeness_from_sums.argtypes = [vp, vp, u64, vp, vp]
     L.blest_get_ms_stats.argtypes = [vp, ctypes.POINTER(u64)]
+    L.blest_closeness_noalloc.argtypes = [vp, vp, u32, vp, vp]
+    L.blest_noalloc_limits.argtypes = [ctypes.POINTER(u32), ctypes.POINTER(u64), ctypes.POINTER(u64)]
     L.blest_l2_microbench.argtypes = [u64, u32, ctypes.POINTER(ctypes.c_double)]
     L.blest_tcgen05_microbench.argtypes = [u32, u32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
     L.blest_get_trace.argtypes = [vp, vp, u32, ctypes.POINTER(u32)]
@@ -266,6 +268,12 @@ class Graph:
                "blest_farness_partial")
         return far_sum, reach_sum
 
+    def closeness_noalloc(self, out, srcs_dev, stream=None):
+        """blest_closeness_noalloc: srcs_dev a CUDA uint32/int32 tensor, out a CUDA float64 tensor; allocates nothing."""
+        k = int(srcs_dev.numel()) if hasattr(srcs_dev, "numel") else int(srcs_dev.size)
+        _check(load().blest_closeness_noalloc(self._h, _ptr(srcs_dev), k, _ptr(out), _stream(stream)), "blest_closeness_noalloc")
+        return out
+
     def ms_stats(self) -> dict:
         """Totals of the last multi-source launch (blest_get_ms_stats)."""
         buf = (ctypes.c_uint64 * 8)()
@@ -348,6 +356,13 @@ def tcgen05_microbench(iters: int = 2048, n: int = 256):
     t, bad = ctypes.c_double(0), ctypes.c_uint64(0)
     _check(load().blest_tcgen05_microbench(int(iters), int(n), ctypes.byref(t), ctypes.byref(bad)), "blest_tcgen05_microbench")
     return t.value, int(bad.value)
+
+
+def noalloc_limits():
+    """(max sources per call, max bytes of one state array, max vertices at kappa = 64) of blest_closeness_noalloc."""
+    a, b, c = ctypes.c_uint32(0), ctypes.c_uint64(0), ctypes.c_uint64(0)
+    _check(load().blest_noalloc_limits(ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)), "blest_noalloc_limits")
+    return int(a.value), int(b.value), int(c.value)
 
 
 def barrier_microbench(iters: int = 2000) -> float:

@@ -968,6 +968,32 @@ int blest_closeness_from_sums(const uint64_t* far_sum, const uint32_t* reach_sum
   return BLEST_OK;
 }
 
+int blest_closeness_noalloc(blest_handle_t h, const uint32_t* srcs_dev, uint32_t n_srcs, double* out_dev, void* cuda_stream) {
+  if (!h || !srcs_dev || !out_dev || n_srcs == 0) return BLEST_EINVAL;
+  if (h->hostOnly) return BLEST_EUNSUPPORTED;
+  // limits of the file-scope scratch (msbfs_kernels.cu): rejected, never truncated
+  const uint64_t stateBytes = (uint64_t)h->rho * 8u * (uint64_t)(h->opt.kappa / 32) * 4u;  // exactly what the kernel touches
+  if (n_srcs > NOALLOC_MAX_SRCS || stateBytes > NOALLOC_MAX_STATE_BYTES || h->Ns > NOALLOC_MAX_SETS) return BLEST_ERANGE;
+  if (!is_device_ptr(srcs_dev) || !is_device_ptr(out_dev)) return BLEST_EINVAL;
+  if (int rc = pending_status(h)) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  persist_use(h, 0);  // (a device limit, not an allocation; only handles that hold a reference touch it)
+  MsParams p{};
+  fill_ms_params(h, p);  // graph arrays, work queues and control block of the handle: allocated by blest_build
+  h->lastCtrl = h->dCtrl;
+  cudaError_t e = cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st);
+  if (e == cudaSuccess) e = launch_closeness_noalloc(p, srcs_dev, n_srcs, h->gridMs, out_dev, st);
+  if (e != cudaSuccess) return ms_fail(e);
+  return BLEST_OK;
+}
+
+int blest_noalloc_limits(uint32_t* max_srcs, uint64_t* max_state_bytes, uint64_t* max_vertices_at_kappa64) {
+  if (max_srcs) *max_srcs = NOALLOC_MAX_SRCS;
+  if (max_state_bytes) *max_state_bytes = NOALLOC_MAX_STATE_BYTES;
+  if (max_vertices_at_kappa64) *max_vertices_at_kappa64 = NOALLOC_MAX_STATE_BYTES / 8u;
+  return BLEST_OK;
+}
+
 int blest_get_ms_stats(blest_handle_t h, uint64_t* out8) {
   if (!h || !out8) return BLEST_EINVAL;
   if (h->hostOnly) return BLEST_EUNSUPPORTED;

@@ -112,4 +112,13 @@ int max_coop_blocks_lazy();
 int max_coop_blocks_eager();
 int max_coop_blocks_msbfs();
 
+// ---- allocation-free closeness of a source subset (blest_closeness_noalloc; msbfs_kernels.cu) ----------------------
+constexpr uint32_t NOALLOC_MAX_SRCS = 4096;             // sources per call
+constexpr uint64_t NOALLOC_MAX_STATE_BYTES = 2u << 20;  // bytes of ONE kappa-bit state array: ceil(n/8) * 8 * kappa/8
+constexpr uint64_t NOALLOC_MAX_SETS = 1u << 16;         // slice sets (one dirty byte each): n <= 524 288
+// p: everything but F / Vc / Vn / dirty / srcs / farS / reachS / stats, which are placed in the file-scope scratch
+// array here.  srcsDev: device uint32[nsrcs] (ids >= n are clamped to n - 1 instead of faulting).  out: device fp64[nsrcs].
+cudaError_t launch_closeness_noalloc(MsParams p, const uint32_t* srcsDev, uint32_t nsrcs, int gridBlocks, double* out,
+                                     cudaStream_t st);
+
 }  // namespace blest

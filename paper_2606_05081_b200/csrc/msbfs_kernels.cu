@@ -10,6 +10,8 @@
 // instances at once as M = OR_{j in mask} F_curr^kappa[column j]  (8 selected ORs of kappa-bit words per slice).
 // The per-instance loop, and with it activeSets, disappears; the per-set OR "A" of Alg. 5 line 51
 // still decides which slice sets are enqueued.  dirtySets is kept as in the paper.
+#include <mutex>
+
 #include "bfs_kernels.cuh"
 
 namespace blest {
@@ -394,6 +396,87 @@ cudaError_t launch_closeness_finalize(uint32_t n, uint32_t rho, const uint32_t* 
   closeness_finalize_kernel<<<blocks > 0 ? blocks : 1, threads, 0, st>>>(n, rho, perm, farT, reachT, farS, reachS, nsrcs, cc,
                                                                           farOut, reachOut);
   return cudaGetLastError();
+}
+
+// ---- allocation-free entry (blest_closeness_noalloc) ---------------------------------------------------------------
+// Some callers cannot allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.
+// For them the scratch of ONE multi-source call lives in this file-scope device array (about 6.2 MiB, held by every GPU
+// that loads the library until the process exits):
+//   [ F | Vc | Vn ]   3 x NOALLOC_MAX_STATE_BYTES   the kappa-bit state arrays
+//   [ dirty ]         NOALLOC_MAX_SETS bytes        dirtySets
+//   [ farS ]          NOALLOC_MAX_SRCS x 8          per-source farness   (must start at zero)
+//   [ reachS ]        NOALLOC_MAX_SRCS x 4          per-source reach     (must start at zero)
+//   [ srcs ]          NOALLOC_MAX_SRCS x 4          sanitised copy of the caller's source ids
+// All calls of the process share it and it keeps the last call's contents: dirty / farS / reachS are cleared at the
+// start of every call (stream-ordered memsets), F / Vc / Vn are cleared or written by the kernel before they are read.
+// Two calls that overlap on the GPU (different streams, no ordering) race on it.
+namespace {
+constexpr size_t NA_OFF_F = 0, NA_OFF_VC = NOALLOC_MAX_STATE_BYTES, NA_OFF_VN = 2 * NOALLOC_MAX_STATE_BYTES;
+constexpr size_t NA_OFF_DIRTY = 3 * NOALLOC_MAX_STATE_BYTES;
+constexpr size_t NA_OFF_FAR = NA_OFF_DIRTY + NOALLOC_MAX_SETS;
+constexpr size_t NA_OFF_REACH = NA_OFF_FAR + (size_t)NOALLOC_MAX_SRCS * 8;
+constexpr size_t NA_OFF_SRCS = NA_OFF_REACH + (size_t)NOALLOC_MAX_SRCS * 4;
+constexpr size_t NA_BYTES = NA_OFF_SRCS + (size_t)NOALLOC_MAX_SRCS * 4;
+static_assert(NA_OFF_FAR % 256 == 0 && NA_OFF_REACH % 256 == 0 && NA_OFF_SRCS % 256 == 0, "sub-arrays stay 256-byte aligned");
+
+static __device__ __align__(256) unsigned char g_noallocScratch[NA_BYTES];
+
+// In host code `g_noallocScratch` is a host-side stand-in, not a device address: the address a kernel may use comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+constexpr int NA_MAX_DEVICES = 64;
+std::mutex g_naMutex;
+unsigned char* g_naPtr[NA_MAX_DEVICES] = {};
+
+cudaError_t noalloc_scratch(unsigned char** out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= NA_MAX_DEVICES) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lk(g_naMutex);
+  if (!g_naPtr[dev]) {
+    void* ptr = nullptr;
+    e = cudaGetSymbolAddress(&ptr, g_noallocScratch);
+    if (e != cudaSuccess) return e;
+    g_naPtr[dev] = static_cast<unsigned char*>(ptr);
+  }
+  *out = g_naPtr[dev];
+  return cudaSuccess;
+}
+
+// Sanitised copy of the caller's source ids into the scratch (device code names the array directly).
+__global__ void noalloc_copy_srcs_kernel(const uint32_t* __restrict__ srcs, uint32_t nsrcs, uint32_t n) {
+  uint32_t* dst = reinterpret_cast<uint32_t*>(g_noallocScratch + NA_OFF_SRCS);
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < nsrcs; i += gridDim.x * blockDim.x) dst[i] = min(srcs[i], n - 1u);
+}
+}  // namespace
+
+cudaError_t launch_closeness_noalloc(MsParams p, const uint32_t* srcsDev, uint32_t nsrcs, int gridBlocks, double* out,
+                                     cudaStream_t st) {
+  unsigned char* base = nullptr;
+  cudaError_t e = noalloc_scratch(&base);
+  if (e != cudaSuccess) return e;
+  p.F = reinterpret_cast<uint32_t*>(base + NA_OFF_F);
+  p.Vc = reinterpret_cast<uint32_t*>(base + NA_OFF_VC);
+  p.Vn = reinterpret_cast<uint32_t*>(base + NA_OFF_VN);
+  p.dirty = base + NA_OFF_DIRTY;
+  p.farS = reinterpret_cast<unsigned long long*>(base + NA_OFF_FAR);
+  p.reachS = reinterpret_cast<uint32_t*>(base + NA_OFF_REACH);
+  p.srcs = reinterpret_cast<const uint32_t*>(base + NA_OFF_SRCS);
+  p.srcBase = 0;
+  p.nsrcs = nsrcs;
+  p.farT = nullptr;
+  p.reachT = nullptr;
+  p.levels = nullptr;
+  p.stats = nullptr;
+  // what must start at zero (the array keeps the last call's contents): dirtySets and the per-source sums
+  e = cudaMemsetAsync(base + NA_OFF_DIRTY, 0, NA_OFF_SRCS - NA_OFF_DIRTY, st);
+  if (e != cudaSuccess) return e;
+  noalloc_copy_srcs_kernel<<<(nsrcs + 255) / 256, 256, 0, st>>>(srcsDev, nsrcs, p.n);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  e = launch_msbfs(p, gridBlocks, st);
+  if (e != cudaSuccess) return e;
+  return launch_closeness_finalize(p.n, p.rho, nullptr, nullptr, nullptr, p.farS, p.reachS, nsrcs, out, nullptr, nullptr, st);
 }
 
 int max_coop_blocks_msbfs() {
