@@ -197,12 +197,17 @@ def ms_alg_bytes(stats: dict, kappa: int, n_slice_sets: int, n: int, accumulate:
     Stage 2, per level: the dirtySets sweep (1 B per slice set); per dirty slice set: 8 rows x (V_next + V_curr read,
       F_curr + V_curr written: 4 KB) + 8 B setPtr + a queue entry per 32 quads (counted with Stage 1) + 12 B per row of
       far / reach accumulation;
-    per batch: V_curr and V_next cleared (2 x n KB)."""
+    pull level (ms_pull_level: Stage 1 + 2 fused, no queue, no dirtySets): every row's visited word read and frontier
+      word written (2 KB per row); per row some live source has not reached: 8 B of row pointers; per neighbour read:
+      4 B column index + its frontier word (KB);
+    per batch: V_curr and V_next cleared (2 x n KB; 3 x with pull levels enabled: F_curr too)."""
     kb = kappa // 8
+    pull_levels = stats.get("pull_levels", 0)
     w = stats["entries"] * (8 + 8 * kb) + stats["quads"] * 20 + stats["probes"] * kb + stats["fresh"] * (kb + 1)
-    w += (stats["levels"] + stats["batches"]) * n_slice_sets
+    w += (stats["levels"] - pull_levels + stats["batches"]) * n_slice_sets
     w += stats["dirty_sets"] * (8 * 4 * kb + 8 + (8 * 12 if accumulate else 0))
-    w += stats["batches"] * 2 * n * kb
+    w += pull_levels * 2 * n * kb + stats.get("pull_rows", 0) * 8 + stats.get("pull_neighbours", 0) * (4 + kb)
+    w += stats["batches"] * (3 if pull_levels else 2) * n * kb
     return int(w)
 
 
@@ -400,7 +405,7 @@ def closeness_measure(args, torch, blest, rank, world, dist, steps, warmup, want
     whole source set once.  N = 1: one blest_closeness call.  N > 1: rank r runs blest_farness_partial over its source
     range, one all-reduce sums the partial target-side arrays, blest_closeness_from_sums divides."""
     n, rp, ci = load_graph("c5_rmat18", args.shrink, rank, world) if args.config == "c5_rmat18" else gg.make_config("c5_rmat18", args.shrink)
-    g = blest.Graph(n, rp, ci, reorder="none", kappa=args.kappa)
+    g = blest.Graph(n, rp, ci, reorder="none", kappa=args.kappa, ms_pull=not args.no_ms_pull)
     info = g.info()
     stream = torch.cuda.current_stream() if world > 1 else torch.cuda.Stream()
     cc = torch.zeros(n, dtype=torch.float64, device="cuda")
@@ -434,6 +439,8 @@ def closeness_measure(args, torch, blest, rank, world, dist, steps, warmup, want
             step(cc)
         barrier()
         stats = g.ms_stats()
+        stats.update({k: v for k, v in g.ms_phases().items() if k.startswith("pull_")})
+        phases = {k: v for k, v in g.ms_phases().items() if k.endswith("_ns")}
         sampler = ClockSampler(int(os.environ.get("LOCAL_RANK", "0"))) if rank == 0 else None
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
@@ -468,7 +475,10 @@ def closeness_measure(args, torch, blest, rank, world, dist, steps, warmup, want
                        "l2": "L2-resident graph (the workload re-traverses a 40 MB graph; no flush)",
                        "bvss_bytes": int(info.bvss_bytes),
                        "parallelism": "sources partitioned over ranks + all-reduce of the target-side sums" if world > 1 else "1 GPU",
-                       "levels_per_batch": stats["levels"] / max(stats["batches"], 1), "vss_entries_per_step": stats["entries"]},
+                       "levels_per_batch": stats["levels"] / max(stats["batches"], 1), "vss_entries_per_step": stats["entries"],
+                       "pull_levels_per_batch": stats.get("pull_levels", 0) / max(stats["batches"], 1),
+                       "pull_neighbours_per_step": stats.get("pull_neighbours", 0),
+                       "phase_ms_cta0": {k[:-3]: round(v / 1e6, 2) for k, v in phases.items()}},
             "roofline": {"bound": "l2", "achieved": achieved, "peak": l2_peak, "unit": "GB/s",
                          "frac": (achieved / l2_peak) if achieved else None, "traffic": None,
                          "peak_source": "measured: blest_l2_microbench (48 MB footprint copy, persistent launch configuration)",
@@ -504,6 +514,7 @@ def main():
     ap.add_argument("--reorder", default=None)
     ap.add_argument("--kappa", type=int, default=64)
     ap.add_argument("--tma-tiles", action="store_true", help="options.tune[0]: TMA-staged slice tiles in the balanced phase")
+    ap.add_argument("--no-ms-pull", action="store_true", help="options.tune[1]: the multi-source kernel never switches to pull levels")
     ap.add_argument("--no-persist", action="store_true", help="options.persist_l2 = off: internal-id levels + gather hand-off")
     ap.add_argument("--keep-trace", action="store_true", help="leave the per-level trace on inside the timed region")
     args = ap.parse_args()

@@ -101,7 +101,8 @@ typedef struct {
   int tune[4];     /* experiment switches of the kernels, 0 = default: [0] = 1: the balanced top-down phase stages its
                       slice tiles in shared memory with TMA bulk copies (cp.async.bulk + mbarrier, two stages per warp)
                       instead of 128-bit loads into registers -- measured 14 % slower on config 4, hence off by default
-                      (DESIGN.md §6); [1..3] unused */
+                      (DESIGN.md §6); [1] = 1: the multi-source kernel never switches a batch to pull levels;
+                      [2..3] unused */
   int reserved[6]; /* [0]: switching == 5 ("scripted", tests): level l runs bottom-up iff bit min(l,31) is set;
                       [1..5]: tuning overrides of the switch cost model in 0.01 ps per unit (top-down edge, top-down
                       vertex, bottom-up vertex, bottom-up scanned neighbour, bottom-up bitmap word); 0 = default */
@@ -201,9 +202,21 @@ int blest_closeness_noalloc(blest_handle_t h, const uint32_t *srcs_dev, uint32_t
 int blest_noalloc_limits(uint32_t *max_srcs, uint64_t *max_state_bytes, uint64_t *max_vertices_at_kappa64);
 
 /* Totals of the most recent multi-source launch, for the roofline (needs options.trace): out8[0] work-queue entries
- * (VSS chunks) consumed by Stage 1, [1] quads they hold, [2] slices whose V_next word was probed, [3] row words updated
- * by an atomic, [4] dirty slice sets swept by Stage 2, [5] levels, [6] source batches, [7] 0.  Synchronises the device. */
+ * (VSS chunks) consumed by Stage 1, [1] quads they hold, [2] slices with a non-zero selection (V_next probed), [3] row words updated
+ * by an atomic, [4] dirty slice sets swept by Stage 2, [5] levels (top-down and pull), [6] source batches, [7] neighbours
+ * read by the pull levels.  Synchronises the device. */
 int blest_get_ms_stats(blest_handle_t h, uint64_t *out8);
+/* Where the most recent multi-source launch spent its time (needs options.trace), in nanoseconds of %globaltimer as seen
+ * by thread 0 of CTA 0, summed over all batches and levels: out8[0] per-batch init (state clears, source bits, level-0
+ * sweep, their barriers), [1] Stage 1 own work, [2] wait at the barrier after Stage 1, [3] Stage 2
+ * own work, [4] wait at the barrier after Stage 2, [5] rows a pull level scanned (some live source not
+ * there yet), [6] pull levels, [7] 0; a pull level's own work counts under [1], its barrier under [2].  Synchronises the device. */
+int blest_get_ms_phases(blest_handle_t h, uint64_t *out8);
+/* Per-level record of the first levels (at most 60, over consecutive batches) of the most recent multi-source launch
+ * (needs options.trace): four words per level -- (level << 32 | work-queue entries consumed), ns of Stage 1 + its
+ * barrier, ns of Stage 2 + its barrier, entries enqueued for the next level -- as thread 0 of CTA 0 sees them.
+ * `out` has room for 4 * max_levels words; *n_levels = records written.  Synchronises the device. */
+int blest_get_ms_level_trace(blest_handle_t h, uint64_t *out, uint32_t max_levels, uint32_t *n_levels);
 
 int blest_get_info(blest_handle_t h, blest_info_t *info);
 

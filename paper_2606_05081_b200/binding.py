@@ -70,7 +70,7 @@ TRACE_DTYPE = np.dtype([("level", "<u4"), ("mode", "<u4"), ("q_entries", "<u4"),
                         ("t_ns", "<u8"), ("t_stage1_ns", "<u8")])
 
 EXPORTS = ["blest_build", "blest_preprocess_host", "blest_configure", "blest_get_call_stats", "blest_bfs", "blest_msbfs", "blest_closeness", "blest_farness",
-           "blest_get_info", "blest_last_status", "blest_farness_partial", "blest_closeness_from_sums", "blest_get_ms_stats",
+           "blest_get_info", "blest_last_status", "blest_farness_partial", "blest_closeness_from_sums", "blest_get_ms_stats", "blest_get_ms_phases", "blest_get_ms_level_trace",
            "blest_l2_microbench", "blest_tcgen05_microbench", "blest_closeness_noalloc", "blest_noalloc_limits", "blest_get_trace", "blest_get_array", "blest_get_vi", "blest_contraction_selftest",
            "blest_mma_microbench", "blest_barrier_microbench", "blest_destroy", "blest_strerror",
            "blest_last_cuda_error"]
@@ -102,6 +102,8 @@ def load(build_if_missing: bool = True):
     L.blest_farness_partial.argtypes = [vp, u32, u32, vp, vp, vp]
     L.blest_closeness_from_sums.argtypes = [vp, vp, u64, vp, vp]
     L.blest_get_ms_stats.argtypes = [vp, ctypes.POINTER(u64)]
+    L.blest_get_ms_phases.argtypes = [vp, ctypes.POINTER(u64)]
+    L.blest_get_ms_level_trace.argtypes = [vp, ctypes.POINTER(u64), ctypes.c_uint32, ctypes.POINTER(ctypes.c_uint32)]
     L.blest_closeness_noalloc.argtypes = [vp, vp, u32, vp, vp]
     L.blest_noalloc_limits.argtypes = [ctypes.POINTER(u32), ctypes.POINTER(u64), ctypes.POINTER(u64)]
     L.blest_l2_microbench.argtypes = [u64, u32, ctypes.POINTER(ctypes.c_double)]
@@ -155,7 +157,7 @@ def _stream(stream):
 
 def _options(reorder="none", builder=0, validate=False, kernel="auto", switching="auto", contraction="auto", kappa=64,
              trace=True, eta=0.0, gamma=0.0, bu_mask=0, costs=None, persist_l2=True, prune_components=True,
-             queue_capacity=0, tma_tiles=False) -> _Options:
+             queue_capacity=0, tma_tiles=False, ms_pull=True) -> _Options:
     o = _Options()
     o.reorder = REORDER[reorder] if isinstance(reorder, str) else int(reorder)
     o.builder = int(builder)
@@ -171,6 +173,7 @@ def _options(reorder="none", builder=0, validate=False, kernel="auto", switching
     o.prune_components = 0 if prune_components else 1
     o.queue_capacity = int(queue_capacity)
     o.tune[0] = int(bool(tma_tiles))
+    o.tune[1] = 0 if ms_pull else 1
     o.reserved[0] = int(bu_mask)
     for k, c in enumerate(costs or ()):  # switch cost model overrides, ps per unit (tuning only): td_edge, td_vertex,
         o.reserved[1 + k] = int(round(100 * float(c)))  # bu_vertex, bu_scan, bu_word
@@ -278,8 +281,24 @@ class Graph:
         """Totals of the last multi-source launch (blest_get_ms_stats)."""
         buf = (ctypes.c_uint64 * 8)()
         _check(load().blest_get_ms_stats(self._h, buf), "blest_get_ms_stats")
-        keys = ("entries", "quads", "probes", "fresh", "dirty_sets", "levels", "batches")
+        keys = ("entries", "quads", "probes", "fresh", "dirty_sets", "levels", "batches", "pull_neighbours")
         return {k: int(buf[i]) for i, k in enumerate(keys)}
+
+    def ms_phases(self) -> dict:
+        """Nanoseconds CTA 0 spent per phase of the last multi-source launch (blest_get_ms_phases)."""
+        buf = (ctypes.c_uint64 * 8)()
+        _check(load().blest_get_ms_phases(self._h, buf), "blest_get_ms_phases")
+        keys = ("init_ns", "stage1_ns", "barrier1_ns", "stage2_ns", "barrier2_ns", "pull_rows", "pull_levels")
+        return {k: int(buf[i]) for i, k in enumerate(keys)}
+
+    def ms_level_trace(self, max_levels: int = 60) -> list:
+        """Per-level records of the first levels of the last multi-source launch (blest_get_ms_level_trace)."""
+        buf = (ctypes.c_uint64 * (4 * max_levels))()
+        k = ctypes.c_uint32(0)
+        _check(load().blest_get_ms_level_trace(self._h, buf, max_levels, ctypes.byref(k)), "blest_get_ms_level_trace")
+        return [{"level": int((buf[4 * i] >> 32) & 0x7FFFFFFF), "pull": bool(buf[4 * i] >> 63),
+                 "entries": int(buf[4 * i] & 0xFFFFFFFF), "stage1_ns": int(buf[4 * i + 1]),
+                 "stage2_ns": int(buf[4 * i + 2]), "enqueued": int(buf[4 * i + 3])} for i in range(k.value)]
 
     # -- introspection
     def info(self) -> Info:

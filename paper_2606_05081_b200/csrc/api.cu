@@ -82,14 +82,15 @@ struct blest_graph {
   int32_t *dL = nullptr, *dStamp = nullptr, *dOut = nullptr;
   // multi-source workspace: grow-only (sized for the widest kappa used so far; a wider kappa frees and re-allocates)
   uint64_t msWords = 0;
-  uint32_t *dMsF = nullptr, *dMsVc = nullptr, *dMsVn = nullptr;
+  uint32_t *dMsF = nullptr, *dMsVc = nullptr, *dMsVn = nullptr, *dMsF2 = nullptr, *dMsLive = nullptr;
   // pinned staging slots for host `srcs` arrays (consumed before the call returns; recycled once their copy has run)
   struct StageSlot { void* host = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; };
   std::vector<StageSlot> stage;
   uint8_t* dDirty = nullptr;
   unsigned long long* dFarT = nullptr;
   uint32_t* dReachT = nullptr;
-  unsigned long long* dMsStats = nullptr;  // [8] totals of the last multi-source launch (blest_get_ms_stats)
+  unsigned long long* dMsStats = nullptr;  // [16] totals of the last multi-source launch (blest_get_ms_stats) + phase times
+                                           // of CTA 0 in [8..15] (blest_get_ms_phases)
   uint64_t wsBytes = 0;
   std::vector<void*> allocs;
 };
@@ -747,24 +748,26 @@ static int ensure_ms_workspace(blest_graph* g) {
     // by enqueued work, hence the synchronisation -- this happens at most three times in a handle's life)
     if (g->dMsF) {
       CK(cudaDeviceSynchronize());
-      for (uint32_t* old : {g->dMsF, g->dMsVc, g->dMsVn}) {
+      for (uint32_t* old : {g->dMsF, g->dMsVc, g->dMsVn, g->dMsF2}) {
         auto it = std::find(g->allocs.begin(), g->allocs.end(), (void*)old);
         if (it != g->allocs.end()) g->allocs.erase(it);
         cudaFree(old);
       }
-      g->wsBytes -= 3 * ((g->msWords * 4 + 15) & ~15ull);
-      g->dMsF = g->dMsVc = g->dMsVn = nullptr;
+      g->wsBytes -= 4 * ((g->msWords * 4 + 15) & ~15ull);
+      g->dMsF = g->dMsVc = g->dMsVn = g->dMsF2 = nullptr;
       g->msWords = 0;
     }
     if ((rc = dev_alloc(g, &g->dMsF, words, true))) return rc;
     if ((rc = dev_alloc(g, &g->dMsVc, words, true))) return rc;
     if ((rc = dev_alloc(g, &g->dMsVn, words, true))) return rc;
+    if ((rc = dev_alloc(g, &g->dMsF2, words, true))) return rc;
     g->msWords = words;
   }
   if (!g->dDirty && (rc = dev_alloc(g, &g->dDirty, (uint64_t)g->Ns + 16, true))) return rc;
   if (!g->dFarT && (rc = dev_alloc(g, &g->dFarT, (uint64_t)g->rho * 8u, true))) return rc;
   if (!g->dReachT && (rc = dev_alloc(g, &g->dReachT, (uint64_t)g->rho * 8u, true))) return rc;
-  if (!g->dMsStats && (rc = dev_alloc(g, &g->dMsStats, 8, true))) return rc;
+  if (!g->dMsStats && (rc = dev_alloc(g, &g->dMsStats, MS_STATS_WORDS, true))) return rc;
+  if (!g->dMsLive && (rc = dev_alloc(g, &g->dMsLive, 24, true))) return rc;
   return BLEST_OK;
 }
 
@@ -779,6 +782,10 @@ static void fill_ms_params(blest_graph* h, MsParams& p) {
   p.hostStatus = h->hStatus;
   p.kappa = h->opt.kappa;
   p.stats = h->opt.trace != 2 ? h->dMsStats : nullptr;
+  // pull levels (target-side accumulation on a symmetric graph only; the kernel checks the rest): a batch switches when a
+  // level's queue holds at least half of all VSSs, i.e. the frontier touches most slice sets; options.tune[1] = 1: never
+  p.F2 = h->dMsF2; p.rowptr = h->dRowptr; p.colidx = h->dColidx; p.live = h->dMsLive;
+  p.pullMin = (h->opt.tune[1] == 1 || h->directed) ? 0u : std::max(1u, h->Nv / 2u);
 }
 
 // Stream-ordered temporaries of one multi-source call: device buffers from the stream's memory pool
@@ -857,7 +864,7 @@ int blest_msbfs(blest_handle_t h, const uint32_t* srcs, uint32_t k, int32_t* lev
   p.levels = devOut ? levels_out : dLevels;
   h->lastCtrl = h->dCtrl;
   if (e == cudaSuccess) e = cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st);
-  if (e == cudaSuccess) e = cudaMemsetAsync(h->dMsStats, 0, 8 * sizeof(unsigned long long), st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->dMsStats, 0, MS_STATS_WORDS * sizeof(unsigned long long), st);
   if (e == cudaSuccess) e = launch_msbfs(p, h->gridMs, st);
   if (e == cudaSuccess && !devOut)
     e = cudaMemcpyAsync(levels_out, dLevels, (size_t)k * h->n * 4, cudaMemcpyDeviceToHost, st);
@@ -912,7 +919,7 @@ static int closeness_impl(blest_handle_t h, const uint32_t* srcs, uint64_t n_src
   if (e == cudaSuccess && reachOut && !reachDev) e = tmp.alloc((void**)&dReachO, n_srcs * 4);
   h->lastCtrl = h->dCtrl;
   if (e == cudaSuccess) e = cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st);
-  if (e == cudaSuccess) e = cudaMemsetAsync(h->dMsStats, 0, 8 * sizeof(unsigned long long), st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->dMsStats, 0, MS_STATS_WORDS * sizeof(unsigned long long), st);
   if (e == cudaSuccess) e = launch_msbfs(p, h->gridMs, st);
   if (e == cudaSuccess)
     e = launch_closeness_finalize(h->n, h->rho, h->hasPerm ? h->dPerm : nullptr, p.farT, p.reachT, p.farS, p.reachS, n_srcs,
@@ -948,7 +955,7 @@ int blest_farness_partial(blest_handle_t h, uint32_t first, uint32_t count, uint
   cudaError_t e = cudaMemsetAsync(h->dFarT, 0, (size_t)h->rho * 8u * 8u, st);
   if (e == cudaSuccess) e = cudaMemsetAsync(h->dReachT, 0, (size_t)h->rho * 8u * 4u, st);
   if (e == cudaSuccess) e = cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st);
-  if (e == cudaSuccess) e = cudaMemsetAsync(h->dMsStats, 0, 8 * sizeof(unsigned long long), st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->dMsStats, 0, MS_STATS_WORDS * sizeof(unsigned long long), st);
   if (e == cudaSuccess) e = launch_msbfs(p, h->gridMs, st);
   // target-side sums in ORIGINAL vertex ids (the finalize kernel maps id -> getVI(perm[id]))
   if (e == cudaSuccess)
@@ -1001,6 +1008,30 @@ int blest_get_ms_stats(blest_handle_t h, uint64_t* out8) {
   if (!h->dMsStats) return BLEST_OK;
   CK(cudaDeviceSynchronize());
   CK(cudaMemcpy(out8, h->dMsStats, 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+  return BLEST_OK;
+}
+
+int blest_get_ms_phases(blest_handle_t h, uint64_t* out8) {
+  if (!h || !out8) return BLEST_EINVAL;
+  if (h->hostOnly) return BLEST_EUNSUPPORTED;
+  for (int k = 0; k < 8; ++k) out8[k] = 0;
+  if (!h->dMsStats) return BLEST_OK;
+  CK(cudaDeviceSynchronize());
+  CK(cudaMemcpy(out8, h->dMsStats + 8, 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+  return BLEST_OK;
+}
+
+int blest_get_ms_level_trace(blest_handle_t h, uint64_t* out, uint32_t max_levels, uint32_t* n_levels) {
+  if (!h || !out || !n_levels) return BLEST_EINVAL;
+  if (h->hostOnly) return BLEST_EUNSUPPORTED;
+  *n_levels = 0;
+  if (!h->dMsStats) return BLEST_OK;
+  CK(cudaDeviceSynchronize());
+  std::vector<uint64_t> buf(MS_STATS_WORDS);
+  CK(cudaMemcpy(buf.data(), h->dMsStats, MS_STATS_WORDS * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+  const uint32_t have = (uint32_t)std::min<uint64_t>(buf[5], MS_TRACE_LEVELS), k = std::min(have, max_levels);
+  for (uint32_t i = 0; i < 4 * k; ++i) out[i] = buf[16 + i];
+  *n_levels = k;
   return BLEST_OK;
 }
 

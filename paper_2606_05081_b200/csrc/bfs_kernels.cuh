@@ -87,8 +87,8 @@ struct MsParams {
   const uint32_t* srcs;  // device, original ids; nullptr = identity (source i = vertex srcBase + i)
   uint64_t srcBase;      // first vertex of the source range when srcs == nullptr (multi-GPU partition)
   uint64_t nsrcs;
-  unsigned long long* stats;  // optional [8]: totals of the launch for the roofline (queue entries, quads, slices probed,
-                              // fresh row updates, dirty slice sets swept, levels, batches)
+  unsigned long long* stats;  // optional [16]: totals of the launch for the roofline (queue entries, quads, slices probed,
+                              // fresh row updates, dirty slice sets swept, levels, batches), [8..12] phase times of CTA 0
   // outputs (any may be nullptr)
   int32_t* levels;              // [nsrcs][n] original ids
   unsigned long long* farT;     // target-side accumulation, indexed by getVI(internal id) (Eq. 7)
@@ -96,7 +96,17 @@ struct MsParams {
   unsigned long long* farS;     // per-source accumulation [nsrcs]
   uint32_t* reachS;
   int kappa;
+  // pull levels (msbfs_kernels.cu ms_pull_level; target-side accumulation only): second frontier array, CSR of the
+  // (relabelled) graph, the rotating live-source masks [3][8] and the queue length from which a batch switches
+  uint32_t* F2;
+  const uint32_t* rowptr;
+  const uint32_t* colidx;
+  uint32_t* live;
+  uint32_t pullMin;  // 0 = never
 };
+constexpr uint32_t MS_TRACE_LEVELS = 60;     // levels recorded by the multi-source kernel's per-level trace
+constexpr size_t MS_STATS_WORDS = 16 + 4 * MS_TRACE_LEVELS;
+
 
 // persistPtr/persistBytes: optional persisting-L2 access-policy window of this launch (levels_out), nullptr/0 = none
 cudaError_t launch_bfs_lazy(const BfsParams& p, int gridBlocks, cudaStream_t st, const void* persistPtr, size_t persistBytes,

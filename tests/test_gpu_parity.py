@@ -427,6 +427,44 @@ def test_closeness_by_source_partition(blest, torch_cuda, reorder):
         assert st["probes"] >= st["fresh"] > 0 and st["dirty_sets"] > 0
 
 
+@pytest.mark.parametrize("kappa", [32, 64, 128, 256])
+def test_msbfs_pull_levels(blest, torch_cuda, kappa):
+    """The pull levels of the multi-source kernel (a batch switches once a level's queue holds half of all VSSs): farness /
+    reach / closeness of every vertex bit-equal to the oracle and to the run that never switches (ms_pull=False); the
+    level trace shows that the switch happened, and only on the all-vertices path."""
+    torch = torch_cuda
+    for maker in (lambda: gg.rmat(11, 12, 5), lambda: gg.disjoint_union(gg.rmat(10, 16, 3), gg.star(70, 0), gg.path(9), gg.empty(3)),
+                  lambda: gg.grid2d(24, 17), lambda: gg.complete(77)):
+        n, rp, ci = maker()
+        far_w, reach_w, cc_w, _ = oracle.closeness(n, rp, ci)
+        got = {}
+        for pull in (True, False):
+            for reorder in ("none", "degree"):
+                with blest.Graph(n, rp, ci, kappa=kappa, ms_pull=pull, reorder=reorder) as g:
+                    far = torch.zeros(n, dtype=torch.int64, device="cuda")
+                    reach = torch.zeros(n, dtype=torch.int32, device="cuda")
+                    cc = torch.zeros(n, dtype=torch.float64, device="cuda")
+                    g.farness(far, reach)
+                    ph, tr = g.ms_phases(), g.ms_level_trace()
+                    g.closeness(cc)
+                    assert g.last_status() == 0
+                    assert np.array_equal(far.cpu().numpy().view(np.uint64), far_w), (pull, reorder)
+                    assert np.array_equal(reach.cpu().numpy().view(np.uint32), reach_w), (pull, reorder)
+                    assert np.array_equal(cc.cpu().numpy(), cc_w), (pull, reorder)
+                    got[(pull, reorder)] = ph["pull_levels"]
+                    assert (ph["pull_levels"] > 0) == any(r["pull"] for r in tr) or len(tr) == 60
+                    if not pull:
+                        assert ph["pull_levels"] == 0 and ph["pull_rows"] == 0
+                    # a source subset counts per source: that path never pulls
+                    sub = np.arange(0, n, 3, dtype=np.uint32)
+                    f2, r2 = np.zeros(sub.size, dtype=np.uint64), np.zeros(sub.size, dtype=np.uint32)
+                    g.farness(f2, r2, srcs=sub)
+                    assert np.array_equal(f2, far_w[sub]) and np.array_equal(r2, reach_w[sub])
+                    assert g.ms_phases()["pull_levels"] == 0
+        if n >= 1000:  # the scale-free graphs reach most slice sets within two levels
+            assert got[(True, "none")] > 0 and got[(True, "degree")] > 0
+
+
 def test_microbenchmarks_run(blest, torch_cuda):
     assert blest.l2_microbench(32 << 20, 10) > 500.0          # GB/s, L2-resident copy
     assert 200.0 < blest.barrier_microbench(500) < 20000.0     # ns per grid barrier
