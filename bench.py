@@ -175,10 +175,13 @@ def w_alg_bytes(trace: np.ndarray, n: int, reach: int, reordered: bool, sweep_wo
                 8 B of row pointers + 4 B per neighbour for the vertices that need the CSR scan);
                 top-down adds 12 B per frontier word consumed (list entry, frontier word, threshold) and the finalisation
                 sweep (12 B per sweep word: V, F_next read, F_stale cleared); bottom-up adds its sweep (8 B per sweep word);
-    per discovered vertex: 4 B level write + 4 B degree (+ 4 B iperm when the graph was reordered)."""
+    per discovered vertex: 4 B level write + 4 B degree (+ 4 B iperm when the graph was reordered); the vertices of the
+                level the pre-fill guessed (trace `reserved` bit 31) cost their degree only."""
     w = 16 * sweep_words + 4 * n + reach * (12 if reordered else 8)
     for r in trace:
         w += int(r["q_bytes"])
+        if int(r["reserved"]) >> 31:  # the level the pre-fill guessed: no level write, no iperm read (degree only)
+            w -= int(r["new_vertices"]) * (8 if reordered else 4)
         if r["mode"] == 1:
             w += 8 * sweep_words
         elif r["mode"] == 2:  # eager kernel (Alg. 2): no sweeps; at least one quad + the queue entry per work item

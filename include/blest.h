@@ -102,7 +102,8 @@ typedef struct {
                       slice tiles in shared memory with TMA bulk copies (cp.async.bulk + mbarrier, two stages per warp)
                       instead of 128-bit loads into registers -- measured 14 % slower on config 4, hence off by default
                       (DESIGN.md §6); [1] = 1: the multi-source kernel never switches a batch to pull levels;
-                      [2..3] unused */
+                      [2] = 1: the lazy kernel always pre-fills levels_out with -1 (no "level guess");
+                      [3] unused */
   int reserved[6]; /* [0]: switching == 5 ("scripted", tests): level l runs bottom-up iff bit min(l,31) is set;
                       [1..5]: tuning overrides of the switch cost model in 0.01 ps per unit (top-down edge, top-down
                       vertex, bottom-up vertex, bottom-up scanned neighbour, bottom-up bitmap word); 0 = default */
@@ -138,7 +139,7 @@ typedef struct {
   uint64_t q_bytes;     /* graph bytes the queue entries cover (20 B per quad, 4 B per edge) */
   uint64_t bu_scanned;  /* bottom-up: neighbours scanned */
   uint32_t unvisited;   /* after this level */
-  uint32_t reserved;
+  uint32_t reserved;    /* bit 31: this level wrote no levels (levels_out was pre-filled with it: the level guess) */
   uint64_t t_ns;        /* %globaltimer at the end of the level, relative to kernel start */
   uint64_t t_stage1_ns; /* %globaltimer after the Stage-1 barrier of this level (lazy kernel), relative to kernel start */
 } blest_level_trace_t;

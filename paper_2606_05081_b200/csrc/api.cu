@@ -68,6 +68,7 @@ struct blest_graph {
   std::vector<uint32_t> deadSrc;  // host bitmap of the vertices of out-degree 0: such a source reaches nothing
   std::vector<uint32_t> hubComp;  // host bitmap of the connected component of the highest-degree vertex
   uint32_t* dOutside = nullptr;   // device bitmap: NOT in that component (zero-degree vertices included)
+  uint32_t* dOutsideOrig = nullptr;  // the same bitmap indexed by ORIGINAL vertex id (reordered graphs; level guess)
   uint32_t nOutsideInSweep = 0;
   uint32_t *dV = nullptr, *dF[3] = {nullptr, nullptr, nullptr}, *dWL[2] = {nullptr, nullptr};
   uint4* dChunks = nullptr;
@@ -500,6 +501,15 @@ static int build_impl(const blest_csr_t* csr, const blest_options_t* optIn, bles
           }
           if ((rc = dev_alloc(g, &g->dOutside, (uint64_t)g->nwords + 16, true))) return rc;
           CK(cudaMemcpy(g->dOutside, outside.data(), (size_t)g->nwords * 4, cudaMemcpyHostToDevice));
+          if (g->hasPerm) {  // by original id: what the pre-fill of levels_out reads (bfs_lazy.cu "level guess")
+            std::vector<uint32_t> oo(g->nwords, 0u);
+            for (uint32_t v = 0; v < g->n; ++v) {
+              const uint32_t u = g->perm[v];
+              if ((outside[u >> 5] >> (u & 31u)) & 1u) oo[v >> 5] |= 1u << (v & 31u);
+            }
+            if ((rc = dev_alloc(g, &g->dOutsideOrig, (uint64_t)g->nwords + 16, true))) return rc;
+            CK(cudaMemcpy(g->dOutsideOrig, oo.data(), (size_t)g->nwords * 4, cudaMemcpyHostToDevice));
+          }
         }
         if ((rc = dev_alloc(g, &g->dPopThr, (uint64_t)g->nwords + 16))) return rc;
         CK(cudaMemcpy(g->dHead, head.data(), (size_t)g->n * sizeof(uint2), cudaMemcpyHostToDevice));
@@ -698,6 +708,11 @@ int blest_bfs(blest_handle_t h, uint32_t src, int32_t* levels_out, void* cuda_st
     p.lvl = p.gather ? h->dL : p.out;
     p.ipermW = (h->hasPerm && !p.gather) ? h->dIperm : nullptr;
     p.srcLvl = p.gather ? p.src : src;
+    // level guess: only when everything the traversal cannot reach is known (source inside the labelled component), as
+    // a bitmap over the indices of p.lvl; options.tune[2] = 1 switches it off
+    p.negBits = nullptr;
+    if (p.isoBits == h->dOutside && h->dOutside && h->opt.tune[2] != 1)
+      p.negBits = (h->hasPerm && !p.gather) ? h->dOutsideOrig : h->dOutside;
     p.ctrl = h->dCtrlLazy;  // self-resetting: no memset node before the launch
     h->lastCtrl = h->dCtrlLazy;
     persist_use(h, usePersist ? bytes : 0);

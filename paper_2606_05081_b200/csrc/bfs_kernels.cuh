@@ -51,6 +51,8 @@ struct BfsParams {
   const uint32_t* ipermW;  // lazy kernel: iperm when lvl is indexed by original ids of a reordered graph, else nullptr
   uint32_t srcLvl;         // index of the source in lvl
   int gather;              // lazy kernel: final pass out[v] = lvl[perm[v]]
+  const uint32_t* negBits; // lazy kernel, level guess: bitmap over the indices of lvl of the vertices this traversal cannot
+                           // reach (everything outside the source's component), or nullptr = no guess (plain -1 pre-fill)
   int32_t* L;      // levels in internal ids (== out when there is no reordering)
   Ctrl* ctrl;
   unsigned int* hostStatus;  // host-mapped latch of the handle (overflow report), may be nullptr

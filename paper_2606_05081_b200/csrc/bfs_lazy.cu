@@ -44,6 +44,10 @@ struct LazyShared {
   uint32_t wlCnt;
   uint32_t wlBase;
   uint32_t buDecision;  // direction of the level, evaluated by the thread that read the control words
+  uint32_t guess;       // the level levels_out is pre-filled with (0 = none; see the kernel)
+  uint32_t guessSlot;   // degree class of the source
+  uint32_t bestLevel;   // (thread 0) the level that discovered the most vertices so far, and how many
+  unsigned long long bestCount;
   // The two directions never run at the same time: the bottom-up lists share their memory with the slice tiles that
   // the balanced top-down phase stages by TMA bulk copies (td_phase_b).
   union {
@@ -523,8 +527,9 @@ __device__ __forceinline__ void td_phase_b(const BfsParams& p, LazyShared& sh, u
 
 // levels_out[original id of u] = level, for the set bits of up to eight words at a time (lane = bit: coalesced
 // iperm / degree loads); also the degree sum of the new frontier for the switch.
+// `store` = false on the level the pre-fill already wrote ("level guess", see the kernel): only the degree sum remains.
 __device__ __forceinline__ void write_levels_dense(const BfsParams& p, uint32_t wordBase, uint32_t fm, uint32_t sel,
-                                                   int32_t level, uint32_t lane, Counters& c) {
+                                                   int32_t level, uint32_t lane, Counters& c, bool store) {
   while (sel) {
     uint32_t u[8], on = 0;
 #pragma unroll
@@ -540,7 +545,7 @@ __device__ __forceinline__ void write_levels_dense(const BfsParams& p, uint32_t 
     }
     uint32_t o[8], dg[8];
 #pragma unroll
-    for (int q = 0; q < 8; ++q) o[q] = ((on >> q) & 1u) ? (p.ipermW ? __ldg(&p.ipermW[u[q]]) : u[q]) : 0u;
+    for (int q = 0; q < 8; ++q) o[q] = (store && ((on >> q) & 1u)) ? (p.ipermW ? __ldg(&p.ipermW[u[q]]) : u[q]) : 0u;
 #pragma unroll
     for (int q = 0; q < 8; ++q) dg[q] = ((on >> q) & 1u) ? __ldg(&p.deg[u[q]]) : 0u;
 #pragma unroll
@@ -548,12 +553,13 @@ __device__ __forceinline__ void write_levels_dense(const BfsParams& p, uint32_t 
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
       BLEST_ASSERT(!((on >> q) & 1u) || (o[q] < p.n && u[q] < p.n));
-      if ((on >> q) & 1u) p.lvl[o[q]] = level;
+      if (store && ((on >> q) & 1u)) p.lvl[o[q]] = level;
     }
   }
 }
 // Same for a lane's own sparse word (a few bits): four vertices in flight.
-__device__ __forceinline__ void write_levels_sparse(const BfsParams& p, uint32_t t, uint32_t bits, int32_t level, Counters& c) {
+__device__ __forceinline__ void write_levels_sparse(const BfsParams& p, uint32_t t, uint32_t bits, int32_t level, Counters& c,
+                                                    bool store) {
   while (bits) {
     uint32_t u[4], o[4];
     bool on[4];
@@ -567,7 +573,7 @@ __device__ __forceinline__ void write_levels_sparse(const BfsParams& p, uint32_t
       }
     }
 #pragma unroll
-    for (int q = 0; q < 4; ++q) o[q] = on[q] ? (p.ipermW ? __ldg(&p.ipermW[u[q]]) : u[q]) : 0u;
+    for (int q = 0; q < 4; ++q) o[q] = (store && on[q]) ? (p.ipermW ? __ldg(&p.ipermW[u[q]]) : u[q]) : 0u;
     uint32_t dg[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) dg[q] = on[q] ? __ldg(&p.deg[u[q]]) : 0u;
@@ -576,14 +582,14 @@ __device__ __forceinline__ void write_levels_sparse(const BfsParams& p, uint32_t
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       BLEST_ASSERT(!on[q] || (o[q] < p.n && u[q] < p.n));
-      if (on[q]) p.lvl[o[q]] = level;
+      if (store && on[q]) p.lvl[o[q]] = level;
     }
   }
 }
 
 // Levels of up to eight (word, bits) entries of the CTA's dense list at a time (lane = bit).
 __device__ __forceinline__ void write_levels_list(const BfsParams& p, const uint2* ent, uint32_t cnt, int32_t level,
-                                                  uint32_t lane, Counters& c) {
+                                                  uint32_t lane, Counters& c, bool store) {
   uint32_t u[8], on = 0;
 #pragma unroll
   for (int q = 0; q < 8; ++q) {
@@ -596,7 +602,7 @@ __device__ __forceinline__ void write_levels_list(const BfsParams& p, const uint
   }
   uint32_t o[8], dg[8];
 #pragma unroll
-  for (int q = 0; q < 8; ++q) o[q] = ((on >> q) & 1u) ? (p.ipermW ? __ldg(&p.ipermW[u[q]]) : u[q]) : 0u;
+  for (int q = 0; q < 8; ++q) o[q] = (store && ((on >> q) & 1u)) ? (p.ipermW ? __ldg(&p.ipermW[u[q]]) : u[q]) : 0u;
 #pragma unroll
   for (int q = 0; q < 8; ++q) dg[q] = ((on >> q) & 1u) ? __ldg(&p.deg[u[q]]) : 0u;
   uint32_t sum = 0;
@@ -606,13 +612,13 @@ __device__ __forceinline__ void write_levels_list(const BfsParams& p, const uint
 #pragma unroll
   for (int q = 0; q < 8; ++q) {
     BLEST_ASSERT(!((on >> q) & 1u) || (o[q] < p.n && u[q] < p.n));
-    if ((on >> q) & 1u) p.lvl[o[q]] = level;
+    if (store && ((on >> q) & 1u)) p.lvl[o[q]] = level;
   }
 }
 
 // Stage 2 after a top-down Stage 1: frontier finalisation (readings R9/R10).
 __device__ __forceinline__ void td_finalize(const BfsParams& p, LazyShared& sh, uint32_t level, uint32_t* Fn, uint32_t* Fs,
-                                            uint32_t* WLn, Ctrl* ctrl, uint32_t ci) {
+                                            uint32_t* WLn, Ctrl* ctrl, uint32_t ci, bool store) {
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + warp, nwarps = gridDim.x * WARPS_PER_BLOCK;
   // Consecutive 32-word batches go to warps of DIFFERENT CTAs (odd multiplier, coprime to the warp count), and the
@@ -655,16 +661,16 @@ __device__ __forceinline__ void td_finalize(const BfsParams& p, LazyShared& sh, 
         BLEST_ASSERT(!dense || base + __popc(dmask & ((1u << lane) - 1u)) < DLIST_CAP);
         if (dense) sh.dlist[base + __popc(dmask & ((1u << lane) - 1u))] = make_uint2(t, fm);
       } else {
-        write_levels_dense(p, wb, fm, dmask, (int32_t)level, lane, c);  // pool full: the owner does them itself
+        write_levels_dense(p, wb, fm, dmask, (int32_t)level, lane, c, store);  // pool full: the owner does them itself
       }
     }
-    if (!dense) write_levels_sparse(p, t, fm, (int32_t)level, c);
+    if (!dense) write_levels_sparse(p, t, fm, (int32_t)level, c, store);
   }
   __syncthreads();
   {
     const uint32_t nd = sh.dvalid;  // entries [0, nd) are valid: reservations are monotone, the first failure ends them
     for (uint32_t e = warp * 8u; e < nd; e += WARPS_PER_BLOCK * 8u)
-      write_levels_list(p, &sh.dlist[e], min(8u, nd - e), (int32_t)level, lane, c);
+      write_levels_list(p, &sh.dlist[e], min(8u, nd - e), (int32_t)level, lane, c, store);
   }
   wl_flush(sh, WLn, &ctrl->wlc[ci]);
   block_accumulate(sh, c, ctrl, ci);
@@ -823,7 +829,7 @@ __device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_
 // V / F_next: they are few), so a level with few unvisited vertices costs one sweep of V plus work proportional to
 // their number.
 __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uint32_t level, const uint32_t* Fp, uint32_t* Fn,
-                                         uint32_t* Fs, uint32_t* WLn, Ctrl* ctrl, uint32_t ci, unsigned long long nu) {
+                                         uint32_t* Fs, uint32_t* WLn, Ctrl* ctrl, uint32_t ci, unsigned long long nu, bool store) {
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + warp, nwarps = gridDim.x * WARPS_PER_BLOCK;
   const uint32_t nSW = p.nSweepWords;
@@ -848,7 +854,8 @@ __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uin
     const uint32_t found = bu_resolve<false>(p, Fp, fshare, slotU, slotTag, lane, u, c, list, listCount);
     uint32_t o[8], dg[8];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) o[k] = ((found >> k) & 1u) ? (p.ipermW ? __ldg(&p.ipermW[u[k] & ~CSR_STAGE]) : (u[k] & ~CSR_STAGE)) : 0u;
+    for (int k = 0; k < 8; ++k)
+      o[k] = (store && ((found >> k) & 1u)) ? (p.ipermW ? __ldg(&p.ipermW[u[k] & ~CSR_STAGE]) : (u[k] & ~CSR_STAGE)) : 0u;
 #pragma unroll
     for (int k = 0; k < 8; ++k) dg[k] = ((found >> k) & 1u) ? __ldg(&p.deg[u[k] & ~CSR_STAGE]) : 0u;
     {
@@ -865,7 +872,7 @@ __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uin
       if ((found >> k) & 1u) {
         const uint32_t uu = u[k] & ~CSR_STAGE, bit = 1u << (uu & 31u);
         BLEST_ASSERT(o[k] < p.n && uu < p.n);
-        p.lvl[o[k]] = (int32_t)level;
+        if (store) p.lvl[o[k]] = (int32_t)level;
         atomicOr(&p.V[uu >> 5], bit);
         oldF[k] = atomicOr(&Fn[uu >> 5], bit);
       }
@@ -907,7 +914,7 @@ __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uin
         const uint32_t found = bu_resolve<true>(p, Fp, fshare, slotU, slotTag, lane, u, c, list, listCount);
         uint32_t o[8], dg[8];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) o[k] = ((found >> k) & 1u) ? (p.ipermW ? __ldg(&p.ipermW[u[k]]) : u[k]) : 0u;
+        for (int k = 0; k < 8; ++k) o[k] = (store && ((found >> k) & 1u)) ? (p.ipermW ? __ldg(&p.ipermW[u[k]]) : u[k]) : 0u;
 #pragma unroll
         for (int k = 0; k < 8; ++k) dg[k] = ((found >> k) & 1u) ? __ldg(&p.deg[u[k]]) : 0u;
         {
@@ -919,7 +926,7 @@ __device__ __forceinline__ void bu_level(const BfsParams& p, LazyShared& sh, uin
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
           BLEST_ASSERT(!((found >> k) & 1u) || (o[k] < p.n && u[k] < p.n));
-          if ((found >> k) & 1u) p.lvl[o[k]] = (int32_t)level;  // lane = bit: coalesced when there is no reordering
+          if (store && ((found >> k) & 1u)) p.lvl[o[k]] = (int32_t)level;  // lane = bit: coalesced when there is no reordering
           const uint32_t fmk = __ballot_sync(FULL, (found >> k) & 1u);
           if (lane == 8u * sub + k) fmw = fmk;
         }
@@ -994,7 +1001,25 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
   // handle (stream-ordered), `epochBase` is where the previous launch left it, and the leader resets the per-call
   // fields below.  Only thread 0 of a CTA evaluates the barrier target, so only it needs the true epoch.
   unsigned int epoch = 0;
-  if (threadIdx.x == 0) epoch = ld_volatile(&ctrl->epochBase);
+  if (threadIdx.x == 0) {
+    epoch = ld_volatile(&ctrl->epochBase);
+    // LEVEL GUESS.  On a low-diameter graph one level discovers most of the component (config 4: level 3 finds 8.8 M of the
+    // 11 M reachable vertices), and its scattered level writes + original-id loads are a third of that level's time.
+    // The previous call on this handle (from a source of similar degree) left the level that discovered the most vertices in
+    // ctrl->guess; this call
+    // pre-fills levels_out with it instead of -1 (the vertices the traversal cannot reach -- p.negBits: everything
+    // outside the source's component, known since blest_build -- still get -1), and the level that equals the guess
+    // then writes no levels at all.  Every other level overwrites the guess as before, and every vertex of the
+    // component is discovered at some level, so the result does not depend on the guess being right.
+    const bool aligned = (((uintptr_t)p.lvl) & 15u) == 0;
+    // (which level that is depends on how far the source is from the hubs: the guess is kept per class of source)
+    const uint32_t sr = __ldg(&p.rowptr[p.src]), sd = __ldg(&p.rowptr[p.src + 1]) - sr;
+    const uint32_t first = sd ? __ldg(&p.colidx[sr]) : 0u;  // lowest id = (after a degree sort) the highest degree
+    sh.guessSlot = (31u - (uint32_t)__clz(sd + 1u)) * 32u + min(31u, 31u - (uint32_t)__clz(first + 1u));
+    sh.guess = (p.negBits && aligned) ? ld_volatile(&ctrl->guess[sh.guessSlot]) : 0u;
+    sh.bestCount = 0;
+    sh.bestLevel = 0;
+  }
   const uint64_t gtid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (uint64_t)gridDim.x * blockDim.x;
   const bool leader = (blockIdx.x == 0 && threadIdx.x == 0);
   if (threadIdx.x < 6) sh.acc[threadIdx.x] = 0;
@@ -1017,8 +1042,32 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     p.F[1][i] = 0;
     p.F[2][i] = 0;
   }
-  // levels = -1 everywhere (reading R1), before any level is written
-  {
+  __syncthreads();
+  // levels = -1 everywhere (reading R1), before any level is written -- or the guessed level where the
+  // traversal can reach
+  if (sh.guess) {
+    const uint32_t guess = sh.guess;
+    uint4* o4 = reinterpret_cast<uint4*>(p.lvl);  // (16-byte aligned: checked above)
+    const uint64_t n4 = (uint64_t)p.n >> 2;
+    for (uint64_t i0 = gtid; i0 < n4; i0 += 4u * nth) {  // four 16-byte stores per round, their bitmap words loaded first
+      uint32_t w[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const uint64_t i = i0 + (uint64_t)q * nth;
+        w[q] = i < n4 ? __ldg(&p.negBits[i >> 3]) : 0u;
+      }
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const uint64_t i = i0 + (uint64_t)q * nth;
+        const uint32_t bits = w[q] >> ((uint32_t)(i & 7u) * 4u);
+        if (i < n4)
+          o4[i] = make_uint4((bits & 1u) ? NONE : guess, (bits & 2u) ? NONE : guess, (bits & 4u) ? NONE : guess,
+                             (bits & 8u) ? NONE : guess);
+      }
+    }
+    const uint64_t v = (n4 << 2) + gtid;
+    if (v < p.n) p.lvl[v] = ((__ldg(&p.negBits[v >> 5]) >> (v & 31u)) & 1u) ? -1 : (int32_t)guess;
+  } else {
     uint32_t* o = reinterpret_cast<uint32_t*>(p.lvl);
     const uint64_t head = min((uint64_t)p.n, (uint64_t)((16u - ((uintptr_t)o & 15u)) & 15u) >> 2);
     const uint64_t n4 = ((uint64_t)p.n - head) >> 2;
@@ -1066,6 +1115,8 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       // the switch (a powf and an expf) is evaluated once per CTA, not by every warp
       const unsigned long long dv = degVisited + sh.ctl[1];
       sh.buDecision = choose_bottom_up(p, level, sh.ctl[0], sh.ctl[1], sh.ctl[2], p.nnz > dv ? p.nnz - dv : 0ull) ? 1u : 0u;
+      // the level that discovered the most vertices so far: the next call's guess (kept in shared memory: no registers)
+      if (level >= 2u && sh.ctl[0] > sh.bestCount) { sh.bestCount = sh.ctl[0]; sh.bestLevel = level - 1u; }
     }
     __syncthreads();
     const unsigned long long nf = sh.ctl[0];
@@ -1074,6 +1125,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     const uint32_t wlCount = (uint32_t)sh.ctl[3];
     const bool bottomUp = sh.buDecision != 0u;
     __syncthreads();
+    const bool storeLv = level != sh.guess;  // the pre-fill already holds this level
     if (nf == 0) break;  // empty frontier ("terminates at the first level with x = 0")
     if (unvAll == 0) break;  // nothing left that could be discovered (everything outside the component is pre-marked)
     degVisited += mf;
@@ -1114,7 +1166,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
           atomicOr(&p.V[v >> 5], bit);
         }
         BLEST_ASSERT(!disc || (o < p.n && v < p.n));
-        if (disc) p.lvl[o] = 1;
+        if (disc && storeLv) p.lvl[o] = 1;
         c.mf += dg;
         c.nnew += disc ? 1u : 0u;
         wl_append(sh, p.WL[1], &ctrl->wlc[ci], v >> 5, disc && old == 0u, lane);
@@ -1129,7 +1181,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       grid_barrier(&ctrl->bar, epoch);
       if (leader) tStage1 = globaltimer();
     } else if (bottomUp) {
-      bu_level(p, sh, level, Fp, Fn, Fs, p.WL[level & 1u], ctrl, ci, nu);
+      bu_level(p, sh, level, Fp, Fn, Fs, p.WL[level & 1u], ctrl, ci, nu, storeLv);
       grid_barrier(&ctrl->bar, epoch);
       if (leader) tStage1 = globaltimer();
     } else {
@@ -1149,7 +1201,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
         grid_barrier(&ctrl->bar, epoch);
       }
       if (leader) tStage1 = globaltimer();
-      td_finalize(p, sh, level, Fn, Fs, p.WL[level & 1u], ctrl, ci);
+      td_finalize(p, sh, level, Fn, Fs, p.WL[level & 1u], ctrl, ci, storeLv);
       grid_barrier(&ctrl->bar, epoch);
     }
     if (leader && p.trace && level - 1 < p.traceCap) {
@@ -1162,7 +1214,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       r.bu_scanned = ld_volatile(&ctrl->buScanned[ci]);
       const unsigned long long ua = ld_volatile(&ctrl->unvisited[ci]);
       r.unvisited = (uint32_t)(ua + p.nIsoInSweep + ((unsigned long long)p.n - min((uint64_t)p.n, (uint64_t)nSW * 32u)));
-      r.reserved = bottomUp ? 0u : ld_volatile(&ctrl->nBig[ci]);
+      r.reserved = (bottomUp ? 0u : ld_volatile(&ctrl->nBig[ci])) | (storeLv ? 0u : 0x80000000u);
       r.t_ns = globaltimer() - ctrl->t0;
       r.t_stage1_ns = tStage1 - ctrl->t0;
       p.trace[level - 1] = r;
@@ -1170,6 +1222,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
   }
   if (leader) {
     ctrl->nlevels = level - 1;
+    ctrl->guess[sh.guessSlot] = sh.bestLevel;
     ctrl->epochBase = epoch;  // every CTA has executed the same barriers: the next launch continues from here
   }
 

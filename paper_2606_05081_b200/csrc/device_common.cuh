@@ -45,6 +45,10 @@ struct Ctrl {
   unsigned int epochBase;           // lazy kernel: grid barriers executed by earlier launches on this control block.  That
                                     // kernel's block is zeroed once at build; every launch resets the per-call fields
                                     // itself and leaves `bar` = epochBase * gridDim (mod 2^32), so no memset precedes a call
+  unsigned int guess[32 * 32];      // lazy kernel: the level that discovered the most vertices in the last call on this handle
+                                    // from a source of the same class (0 = none yet): the next such call pre-fills levels_out
+                                    // with it (bfs_lazy.cu "level guess").  Class = (floor(log2(degree + 1)),
+                                    // floor(log2(internal id of the first neighbour + 1))): how far the source is from the hubs
 };
 
 // Work-queue overflow: flagged in the control block of the call (blest_get_trace) and latched in the handle's

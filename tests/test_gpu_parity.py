@@ -427,6 +427,32 @@ def test_closeness_by_source_partition(blest, torch_cuda, reorder):
         assert st["probes"] >= st["fresh"] > 0 and st["dirty_sets"] > 0
 
 
+@pytest.mark.parametrize("reorder", ["none", "degree", "rcm"])
+def test_level_guess(blest, torch_cuda, reorder):
+    """The lazy kernel pre-fills levels_out with the level that discovered the most vertices in an earlier call from a
+    source of the same class (and -1 where the traversal cannot reach): right or wrong, the result is the oracle's.
+    Sources alternate between hubs, leaves, a far corner of an attached path and other components, so that right
+    guesses, wrong guesses and "no guess" (source outside the labelled component) all occur on one handle."""
+    torch = torch_cuda
+    n, rp, ci = gg.disjoint_union(gg.rmat(12, 12, 77), gg.path(40), gg.star(9, 3), gg.empty(4))
+    deg = np.diff(rp.astype(np.int64))
+    big = int(np.argmax(deg))
+    srcs = [big, int(np.flatnonzero(deg == 1)[0]), 4096 + 39, big, int(np.flatnonzero(deg == 2)[0]), 4096 + 40 + 3, n - 1, big,
+            int(np.flatnonzero(deg == 1)[1]), int(np.flatnonzero(deg == 1)[0])]
+    for guess in (True, False):
+        used = 0
+        with blest.Graph(n, rp, ci, kernel="lazy", reorder=reorder, level_guess=guess) as g:
+            out = torch.full((n,), 5, dtype=torch.int32, device="cuda")
+            for rep in range(2):
+                for s in srcs:
+                    g.bfs(s, out)
+                    assert np.array_equal(out.cpu().numpy(), oracle.bfs(n, rp, ci, s)), (guess, reorder, s)
+                    tr = g.trace()
+                    used += int(np.any(tr["reserved"] >> 31)) if tr.size else 0
+            assert g.last_status() == 0
+        assert (used > 0) == guess
+
+
 @pytest.mark.parametrize("kappa", [32, 64, 128, 256])
 def test_msbfs_pull_levels(blest, torch_cuda, kappa):
     """The pull levels of the multi-source kernel (a batch switches once a level's queue holds half of all VSSs): farness /
