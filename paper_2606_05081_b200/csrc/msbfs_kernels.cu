@@ -79,6 +79,79 @@ __device__ __forceinline__ void red_or_words(uint32_t* base, uint64_t idx, const
   }
 }
 
+// Stage 1 in its first form: one entry at a time, the contraction as a loop over the mask bits.  Kept for kappa = 256,
+// where the pipelined table form below is 8 % slower (32-byte table entries, one slice's probe in flight at a time).
+template <int KW>
+__device__ __forceinline__ void ms_stage1_loop(const MsParams& p, MsShared& sh, const uint2* Qc, uint32_t qcount) {
+  uint32_t* fset = sh.fset[threadIdx.x >> 5];
+  const uint32_t lane = threadIdx.x & 31;
+  const uint32_t gwarp = blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5), nwarps = gridDim.x * WARPS_PER_BLOCK;
+  for (uint32_t i = gwarp; i < qcount; i += nwarps) {
+    BLEST_ASSERT(i < p.qcap);
+    const uint2 e = Qc[i];
+    const uint32_t nq = (e.y & 31u) + 1u, s = e.y >> 5;
+    BLEST_ASSERT(s < p.Ns && (uint64_t)e.x + nq <= p.nQuads);
+    uint4 rows = make_uint4(0, 0, 0, 0);
+    uint32_t m = 0;
+    if (lane < nq) {
+      rows = __ldg(p.rowIds + e.x + lane);
+      m = __ldg(p.masks + e.x + lane);
+    }
+    // the first sigma lanes gather the kappa-bit frontier words of the set's 8 columns into shared
+    // memory; every lane then reads the words its mask bits select (same address across lanes: a broadcast)
+    __syncwarp();
+    if (lane < 8) {
+      uint32_t fv[KW];
+      load_words<KW>(p.F, (uint64_t)lane * p.rho + s, fv);
+#pragma unroll
+      for (int w = 0; w < KW; ++w) fset[lane * KW + w] = fv[w];
+    }
+    __syncwarp();
+    const uint32_t ru[4] = {rows.x, rows.y, rows.z, rows.w};
+    uint32_t nProbe = 0, nFresh = 0;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      const uint32_t mb = (m >> (8 * c)) & 0xFFu;
+      if (mb) {
+        uint32_t M[KW];  // per-row kappa-bit accumulation buffer ("M[0..3]")
+#pragma unroll
+        for (int w = 0; w < KW; ++w) M[w] = 0;
+        for (uint32_t b = mb; b; b &= b - 1) {  // M = OR over the set bits j of the mask of F_curr^kappa[column j]
+          const uint32_t j = (uint32_t)__ffs(b) - 1u;
+#pragma unroll
+          for (int w = 0; w < KW; ++w) M[w] |= fset[j * KW + w];
+        }
+        const uint32_t u = ru[c];
+        BLEST_ASSERT(u < p.n);
+        const uint64_t idx = (uint64_t)(u & 7u) * p.rho + (u >> 3);  // getVI(u, rho)
+        uint32_t any = 0;
+#pragma unroll
+        for (int w = 0; w < KW; ++w) any |= M[w];
+        if (any) {  // one probe and one RED per row, each a single kappa-bit access
+          uint32_t vn[KW], fresh[KW];
+          load_words<KW>(p.Vn, idx, vn);
+          ++nProbe;
+          any = 0;
+#pragma unroll
+          for (int w = 0; w < KW; ++w) { fresh[w] = M[w] & ~vn[w]; any |= fresh[w]; }
+          if (any) {
+            red_or_words<KW>(p.Vn, idx, fresh);
+            p.dirty[u >> 3] = 1;  // PAPER.md:583 dirtySets
+            ++nFresh;
+          }
+        }
+      }
+    }
+    if (p.stats) {
+      const uint32_t tp = __reduce_add_sync(0xffffffffu, nProbe), tf = __reduce_add_sync(0xffffffffu, nFresh);
+      if (lane == 0) {
+        unsigned long long* cnt = sh.cnt[threadIdx.x >> 5];
+        cnt[0] += 1; cnt[1] += nq; cnt[2] += tp; cnt[3] += tf;
+      }
+    }
+  }
+}
+
 // Shared-memory table entry e (a kappa-bit word) of a warp's fset / tab.
 template <int KW>
 __device__ __forceinline__ void tab_load(const uint32_t* tab, uint32_t e, uint32_t (&w)[KW]) {
@@ -258,6 +331,10 @@ __device__ __forceinline__ void publish_live(const MsParams& p, MsShared& sh, co
 // skips them after one coalesced load.  Lane = row (4 consecutive slice sets per warp step: the words of a step are 8 x 32
 // contiguous bytes); rows of up to PULL_SMALL neighbours are scanned by their own lane, longer ones by the whole warp, 64
 // neighbours per round.  A batch switches once (kernel loop) and stays in pull mode: V_next is not maintained here.
+// The groups are assigned statically in natural order.  Measured alternatives on config 5: claiming groups from one
+// global counter, +20 % (13 K same-address atomics per level at about 2.5 ns each); a list ordered by degree sum with the
+// heaviest groups paired with the lightest, +8 % (the heavy groups then run at the same time); the first pull level sits at
+// the rate one SM's L1 forwards scattered sectors (7.6 M frontier words / 148 SMs x 2 cycles = 52 us of its 60 us).
 constexpr uint32_t PULL_SMALL = 8;
 template <int KW>
 __device__ __forceinline__ void ms_pull_level(const MsParams& p, MsShared& sh, uint32_t level, const uint32_t* Fc, uint32_t* Fn) {
@@ -597,7 +674,8 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_co
       ++nLevels;
       if (!PS && p.pullMin && p.live) {
         if (gtid < 8) p.live[((level + 2u) % 3u) * 8u + gtid] = 0;  // the slot the NEXT level accumulates into
-        if (!pull && !p.levels && level >= 2u && qcount >= p.pullMin) pull = true;
+        // (kappa = 256: the pull level's 32-byte words spill at 64 registers per thread and it measures 4 % slower: never)
+        if (KW < 8 && !pull && !p.levels && level >= 2u && qcount >= p.pullMin) pull = true;
       }
       if (!PS && pull) {
         ++nPull;
@@ -619,7 +697,8 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_co
         continue;
       }
       const unsigned long long tl0 = timing ? globaltimer() : 0ull;
-      ms_stage1<KW>(p, sh, p.Q[par], qcount);
+      if (KW == 8) ms_stage1_loop<KW>(p, sh, p.Q[par], qcount);
+      else ms_stage1<KW>(p, sh, p.Q[par], qcount);
       phase(1);
       grid_barrier(&ctrl->bar, epoch);
       phase(2);

@@ -487,7 +487,7 @@ def test_msbfs_pull_levels(blest, torch_cuda, kappa):
                     g.farness(f2, r2, srcs=sub)
                     assert np.array_equal(f2, far_w[sub]) and np.array_equal(r2, reach_w[sub])
                     assert g.ms_phases()["pull_levels"] == 0
-        if n >= 1000:  # the scale-free graphs reach most slice sets within two levels
+        if n >= 1000 and kappa < 256:  # the scale-free graphs reach most slice sets within two levels (kappa = 256 never pulls)
             assert got[(True, "none")] > 0 and got[(True, "degree")] > 0
 
 
