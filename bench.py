@@ -397,6 +397,12 @@ def microbench_extra(blest):
         if hasattr(blest, "tcgen05_microbench"):
             out["tcgen05_i8_tera_bytemacs"] = blest.tcgen05_microbench(2048)[0]
         out["grid_barrier_ns"] = blest.barrier_microbench(2000)
+        for ctas in (8, 16):  # thread-block clusters: barrier and distributed-shared-memory load latency
+            try:
+                b, d = blest.cluster_microbench(ctas, 2000)
+                out[f"cluster{ctas}_barrier_ns"], out[f"cluster{ctas}_dsmem_load_ns"] = b, d
+            except Exception as e:  # a cluster size the device refuses is reported, not fatal
+                out[f"cluster{ctas}_error"] = str(e)
         out["l2_copy_gbs"] = blest.l2_microbench(48 << 20, 50)
     except Exception as e:  # a microbenchmark must not take the headline down
         out["error"] = repr(e)

@@ -267,6 +267,12 @@ int blest_l2_microbench(uint64_t bytes, uint32_t iters, double *gb_per_s);
 /* Grid-barrier latency microbenchmark: `iters` back-to-back grid barriers in the persistent launch configuration. */
 int blest_barrier_microbench(uint32_t iters, double *ns_per_barrier);
 
+/* Thread-block-cluster microbenchmark (the candidate small-frontier mode of DESIGN.md §9): ONE cluster of `cluster_ctas`
+ * (1, 2, 4, 8 or -- non-portable -- 16) CTAs of 1 024 threads executes `iters` back-to-back cluster barriers
+ * (barrier.cluster arrive.release / wait.acquire) and a chain of `iters` dependent loads from the other CTAs' shared memory
+ * (mapa + ld.shared::cluster); nanoseconds per barrier and per load. */
+int blest_cluster_microbench(int cluster_ctas, uint32_t iters, double *ns_per_barrier, double *ns_per_dsmem_load);
+
 void blest_destroy(blest_handle_t h);
 const char *blest_strerror(int status);
 int blest_last_cuda_error(void);

@@ -72,7 +72,7 @@ TRACE_DTYPE = np.dtype([("level", "<u4"), ("mode", "<u4"), ("q_entries", "<u4"),
 EXPORTS = ["blest_build", "blest_preprocess_host", "blest_configure", "blest_get_call_stats", "blest_bfs", "blest_msbfs", "blest_closeness", "blest_farness",
            "blest_get_info", "blest_last_status", "blest_farness_partial", "blest_closeness_from_sums", "blest_get_ms_stats", "blest_get_ms_phases", "blest_get_ms_level_trace",
            "blest_l2_microbench", "blest_tcgen05_microbench", "blest_closeness_noalloc", "blest_noalloc_limits", "blest_get_trace", "blest_get_array", "blest_get_vi", "blest_contraction_selftest",
-           "blest_mma_microbench", "blest_barrier_microbench", "blest_destroy", "blest_strerror",
+           "blest_mma_microbench", "blest_barrier_microbench", "blest_cluster_microbench", "blest_destroy", "blest_strerror",
            "blest_last_cuda_error"]
 
 
@@ -116,6 +116,7 @@ def load(build_if_missing: bool = True):
     L.blest_contraction_selftest.argtypes = [i32, ctypes.POINTER(u64)]
     L.blest_mma_microbench.argtypes = [i32, u32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     L.blest_barrier_microbench.argtypes = [u32, ctypes.POINTER(ctypes.c_double)]
+    L.blest_cluster_microbench.argtypes = [ctypes.c_int, u32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     L.blest_destroy.argtypes = [vp]
     L.blest_destroy.restype = None
     L.blest_strerror.argtypes = [i32]
@@ -383,6 +384,13 @@ def noalloc_limits():
     a, b, c = ctypes.c_uint32(0), ctypes.c_uint64(0), ctypes.c_uint64(0)
     _check(load().blest_noalloc_limits(ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)), "blest_noalloc_limits")
     return int(a.value), int(b.value), int(c.value)
+
+
+def cluster_microbench(cluster_ctas: int = 8, iters: int = 2000):
+    """(ns per cluster barrier, ns per dependent distributed-shared-memory load) for one cluster of `cluster_ctas` CTAs."""
+    a, b = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(load().blest_cluster_microbench(int(cluster_ctas), iters, ctypes.byref(a), ctypes.byref(b)), "blest_cluster_microbench")
+    return a.value, b.value
 
 
 def barrier_microbench(iters: int = 2000) -> float:

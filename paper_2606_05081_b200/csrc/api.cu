@@ -15,6 +15,7 @@ namespace blest {
 cudaError_t run_contraction_selftest(int contraction, unsigned long long* dMismatch);
 cudaError_t run_mma_peak(int kind, uint32_t iters, int blocks, int* dSink, double* macsPerLaunch);
 cudaError_t run_barrier_bench(unsigned int* dBar, uint32_t iters, int blocks, unsigned long long* dNs);
+cudaError_t run_cluster_bench(int clusterCtas, uint32_t iters, unsigned long long* dOut);
 cudaError_t run_l2_copy(const uint4* src, uint4* dst, uint64_t n16, uint32_t iters, int blocks);
 cudaError_t run_tcgen05_peak(uint32_t iters, uint32_t n, int blocks, unsigned int* dBad, double* macsPerLaunch);
 }  // namespace blest
@@ -1207,6 +1208,24 @@ int blest_l2_microbench(uint64_t bytes, uint32_t iters, double* gb_per_s) {
   if (b) cudaFree(b);
   CK(e);
   *gb_per_s = (double)n16 * 32.0 * iters / (best * 1e-3) / 1e9;
+  return BLEST_OK;
+}
+
+int blest_cluster_microbench(int cluster_ctas, uint32_t iters, double* ns_per_barrier, double* ns_per_dsmem_load) {
+  if (!ns_per_barrier || !ns_per_dsmem_load || iters == 0 || cluster_ctas < 1 || cluster_ctas > 16 ||
+      (cluster_ctas & (cluster_ctas - 1)))
+    return BLEST_EINVAL;
+  unsigned long long* dOut = nullptr;
+  CK(cudaMalloc((void**)&dOut, 24));
+  cudaError_t e = cudaMemset(dOut, 0, 24);
+  if (e == cudaSuccess) e = run_cluster_bench(cluster_ctas, iters, dOut);
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  unsigned long long v[3] = {0, 0, 0};
+  if (e == cudaSuccess) e = cudaMemcpy(v, dOut, 24, cudaMemcpyDeviceToHost);
+  cudaFree(dOut);
+  CK(e);
+  *ns_per_barrier = (double)v[0] / iters;
+  *ns_per_dsmem_load = (double)v[1] / iters;
   return BLEST_OK;
 }
 

@@ -192,6 +192,59 @@ cudaError_t run_mma_peak(int kind, uint32_t iters, int blocks, int* dSink, doubl
   return cudaGetLastError();
 }
 
+// Thread-block cluster primitives (the sm_90+/sm_100 feature a small-frontier mode would use): `iters` back-to-back
+// cluster barriers (barrier.cluster.arrive.release + wait.acquire: every thread of every CTA of the cluster) and a chain
+// of `iters` dependent loads from the shared memory of the OTHER CTAs (mapa + ld.shared::cluster), one cluster of 1 024-thread
+// CTAs.  out[0] = ns of the barriers, out[1] = ns of the loads, out[2] = the chain's last value (keeps the loads alive).
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__global__ void __launch_bounds__(BLOCK_THREADS, 1) cluster_bench_kernel(uint32_t iters, unsigned long long* out) {
+  __shared__ uint32_t slot[32];
+  uint32_t rank, nctas;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
+  asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(nctas));
+  if (threadIdx.x < 32) slot[threadIdx.x] = (threadIdx.x * 7u + 1u) & 31u;  // a permutation of 0..31: the chain's next index
+  cluster_sync_all();
+  const unsigned long long t0 = globaltimer();
+  for (uint32_t i = 0; i < iters; ++i) cluster_sync_all();
+  const unsigned long long t1 = globaltimer();
+  if (rank == 0 && threadIdx.x == 0) {
+    uint32_t idx = 0, cta = 1u % nctas;
+    const unsigned long long t2 = globaltimer();
+    for (uint32_t i = 0; i < iters; ++i) {
+      uint32_t remote;
+      asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem_u32(&slot[idx])), "r"(cta));
+      asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(idx) : "r"(remote) : "memory");
+      cta = cta + 1u == nctas ? (nctas > 1u ? 1u : 0u) : cta + 1u;
+    }
+    const unsigned long long t3 = globaltimer();
+    out[0] = t1 - t0;
+    out[1] = t3 - t2;
+    out[2] = idx;
+  }
+  cluster_sync_all();  // no CTA leaves while its shared memory may still be read
+}
+
+cudaError_t run_cluster_bench(int clusterCtas, uint32_t iters, unsigned long long* dOut) {
+  cudaError_t e = cudaSuccess;
+  if (clusterCtas > 8) {
+    e = cudaFuncSetAttribute(cluster_bench_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    if (e != cudaSuccess) return e;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)clusterCtas);
+  cfg.blockDim = dim3(BLOCK_THREADS);
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = (unsigned)clusterCtas;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, cluster_bench_kernel, iters, dOut);
+}
+
 cudaError_t run_barrier_bench(unsigned int* dBar, uint32_t iters, int blocks, unsigned long long* dNs) {
   void* args[] = {(void*)&dBar, (void*)&iters, (void*)&dNs};
   return cudaLaunchCooperativeKernel((const void*)barrier_bench_kernel, dim3(blocks), dim3(BLOCK_THREADS), args, 0, 0);

@@ -18,7 +18,6 @@ namespace blest {
 
 namespace {
 
-constexpr uint32_t NONE = 0xffffffffu;
 
 struct MsShared {
   BigSeg bigList[WARPS_PER_BLOCK][BIG_CAP];

@@ -494,6 +494,9 @@ def test_msbfs_pull_levels(blest, torch_cuda, kappa):
 def test_microbenchmarks_run(blest, torch_cuda):
     assert blest.l2_microbench(32 << 20, 10) > 500.0          # GB/s, L2-resident copy
     assert 200.0 < blest.barrier_microbench(500) < 20000.0     # ns per grid barrier
+    for ctas in (1, 2, 8):                                       # thread-block clusters (portable sizes)
+        b, d = blest.cluster_microbench(ctas, 500)
+        assert 10.0 < b < 20000.0 and 5.0 < d < 20000.0, (ctas, b, d)
     assert blest.mma_microbench("mma_u8", 256)[0] > 10.0
 
 
