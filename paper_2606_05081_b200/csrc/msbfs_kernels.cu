@@ -19,6 +19,10 @@ namespace blest {
 namespace {
 
 
+constexpr uint32_t PULL_SMALL = 8;      // pull level: rows of up to this many neighbours are scanned by their own lane,
+constexpr uint32_t PULL_LONG = 1024;    // longer ones by their warp, rows beyond this by the whole CTA
+constexpr uint32_t PULL_LONG_CAP = 64;  // (per CTA and level; further ones stay with their warp)
+
 struct MsShared {
   BigSeg bigList[WARPS_PER_BLOCK][BIG_CAP];
   uint32_t bigCnt[WARPS_PER_BLOCK];
@@ -30,6 +34,9 @@ struct MsShared {
   unsigned long long tPh[5], tMark;  // phase times of CTA 0 (blest_get_ms_phases)
   uint32_t liveAcc[8];               // OR of the frontier words this CTA produced in the current level (pull levels)
   unsigned int updAcc;               // rows this CTA updated in the current pull level
+  unsigned int longCnt;              // pull level: rows of more than PULL_LONG neighbours met by this CTA ...
+  uint4 longRow[PULL_LONG_CAP];      // ... {row, first, end of its neighbour list, 0}: scanned by the whole CTA
+  uint32_t longAcc[PULL_LONG_CAP][8];  // ... and the OR of the frontier words its warps found
   unsigned long long cnt[WARPS_PER_BLOCK][7];  // per warp (lane 0): queue entries, quads, slices probed, fresh row
                                                // updates, dirty slice sets swept, pull: rows scanned, neighbours read
                                                // -- totals for the roofline (p.stats)
@@ -334,7 +341,6 @@ __device__ __forceinline__ void publish_live(const MsParams& p, MsShared& sh, co
 // global counter, +20 % (13 K same-address atomics per level at about 2.5 ns each); a list ordered by degree sum with the
 // heaviest groups paired with the lightest, +8 % (the heavy groups then run at the same time); the first pull level sits at
 // the rate one SM's L1 forwards scattered sectors (7.6 M frontier words / 148 SMs x 2 cycles = 52 us of its 60 us).
-constexpr uint32_t PULL_SMALL = 8;
 template <int KW>
 __device__ __forceinline__ void ms_pull_level(const MsParams& p, MsShared& sh, uint32_t level, const uint32_t* Fc, uint32_t* Fn) {
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -388,7 +394,17 @@ __device__ __forceinline__ void ms_pull_level(const MsParams& p, MsShared& sh, u
     // longer rows: the whole warp, one row at a time, 128 neighbours per round, until every source the row lacks is
     // covered.  (Concatenating the lists of the group's rows and walking them together, with shared-memory atomics per
     // neighbour, was measured 30-45 % slower on config 5: it gives up the early exit.)
-    uint32_t big = __ballot_sync(0xffffffffu, deg > PULL_SMALL);
+    // (rows beyond PULL_LONG neighbours are left to the whole CTA, below: one warp would need deg / 128 rounds for them --
+    // measured on config 5, first pull level: the slowest CTA took 110 us against a mean of 68)
+    bool deferred = false;
+    if (KW >= 4 && deg > PULL_LONG) {  // (kappa = 64: measured 3 % slower with the CTA phase, kappa = 128: 9 % faster)
+      const uint32_t k = atomicAdd(&sh.longCnt, 1u);
+      if (k < PULL_LONG_CAP) {
+        sh.longRow[k] = make_uint4(u, r0, r1, 0u);
+        deferred = true;
+      }
+    }
+    uint32_t big = __ballot_sync(0xffffffffu, deg > PULL_SMALL && !deferred);
     while (big) {
       const int src = __ffs(big) - 1;
       big &= big - 1;
@@ -428,7 +444,7 @@ __device__ __forceinline__ void ms_pull_level(const MsParams& p, MsShared& sh, u
         for (int w = 0; w < KW; ++w) acc[w] = red[w];
       }
     }
-    if (valid) {
+    if (valid && !deferred) {
       uint32_t nw[KW], anyNew = 0, pc = 0;
 #pragma unroll
       for (int w = 0; w < KW; ++w) { nw[w] = acc[w] & need[w]; anyNew |= nw[w]; pc += __popc(nw[w]); lv[w] |= nw[w]; }
@@ -442,6 +458,75 @@ __device__ __forceinline__ void ms_pull_level(const MsParams& p, MsShared& sh, u
         ++nUpd;
       }
     }
+  }
+  // the CTA's long rows: every warp scans a 128-neighbour share per round, the partial ORs meet in shared memory, one
+  // thread per row finalises it
+  if (KW >= 4) {
+    __syncthreads();
+    const uint32_t nLong = min(sh.longCnt, PULL_LONG_CAP);
+    for (uint32_t i = 0; i < nLong; ++i) {
+      const uint4 row = sh.longRow[i];
+      uint32_t a[KW], nd[KW];
+      {
+        uint32_t vc[KW];
+        load_words<KW>(p.Vc, (uint64_t)(row.x & 7u) * rho + (row.x >> 3), vc);  // (one address per warp: a broadcast)
+#pragma unroll
+        for (int w = 0; w < KW; ++w) { nd[w] = live[w] & ~vc[w]; a[w] = 0; }
+      }
+      for (uint32_t k = row.y + warp * 128u; k < row.z; k += WARPS_PER_BLOCK * 128u) {
+        {  // stop as soon as the warps together have covered every source the row lacks
+          uint32_t lack = 0;
+#pragma unroll
+          for (int w = 0; w < KW; ++w) lack |= nd[w] & ~*(volatile uint32_t*)&sh.longAcc[i][w];
+          if (!lack) break;
+        }
+        uint32_t f0[KW], f1[KW], f2[KW], f3[KW];
+#pragma unroll
+        for (int w = 0; w < KW; ++w) f0[w] = f1[w] = f2[w] = f3[w] = 0;
+        const uint32_t k0 = k + lane, k1 = k + 32u + lane, k2 = k + 64u + lane, k3 = k + 96u + lane;
+        uint32_t v0 = 0, v1 = 0, v2 = 0, v3 = 0;
+        if (k0 < row.z) v0 = __ldg(&p.colidx[k0]);
+        if (k1 < row.z) v1 = __ldg(&p.colidx[k1]);
+        if (k2 < row.z) v2 = __ldg(&p.colidx[k2]);
+        if (k3 < row.z) v3 = __ldg(&p.colidx[k3]);
+        BLEST_ASSERT(v0 < p.n && v1 < p.n && v2 < p.n && v3 < p.n);
+        if (k0 < row.z) load_words<KW>(Fc, (uint64_t)(v0 & 7u) * rho + (v0 >> 3), f0);
+        if (k1 < row.z) load_words<KW>(Fc, (uint64_t)(v1 & 7u) * rho + (v1 >> 3), f1);
+        if (k2 < row.z) load_words<KW>(Fc, (uint64_t)(v2 & 7u) * rho + (v2 >> 3), f2);
+        if (k3 < row.z) load_words<KW>(Fc, (uint64_t)(v3 & 7u) * rho + (v3 >> 3), f3);
+#pragma unroll
+        for (int w = 0; w < KW; ++w) {
+          a[w] = (f0[w] | f1[w] | f2[w] | f3[w]) & nd[w];
+          const uint32_t r = __reduce_or_sync(0xffffffffu, a[w]);
+          if (lane == 0 && r) atomicOr(&sh.longAcc[i][w], r);
+        }
+        if (lane == 0) nNbr += min(128u, row.z - k);
+      }
+    }
+    __syncthreads();
+    if (threadIdx.x < nLong) {
+      const uint4 row = sh.longRow[threadIdx.x];
+      const uint64_t idx = (uint64_t)(row.x & 7u) * rho + (row.x >> 3);
+      uint32_t vc[KW], nw[KW], anyNew = 0, pc = 0;
+      load_words<KW>(p.Vc, idx, vc);
+#pragma unroll
+      for (int w = 0; w < KW; ++w) {
+        nw[w] = sh.longAcc[threadIdx.x][w] & live[w] & ~vc[w];
+        sh.longAcc[threadIdx.x][w] = 0;
+        anyNew |= nw[w]; pc += __popc(nw[w]); lv[w] |= nw[w];
+      }
+      store_words<KW>(Fn, idx, nw);
+      if (anyNew) {
+#pragma unroll
+        for (int w = 0; w < KW; ++w) vc[w] |= nw[w];
+        store_words<KW>(p.Vc, idx, vc);
+        if (p.farT) p.farT[idx] += (unsigned long long)level * pc;
+        if (p.reachT) p.reachT[idx] += pc;
+        ++nUpd;
+      }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) sh.longCnt = 0;
   }
   // the level's termination test is the queue tail (kernel loop): it advances by the number of rows updated
   {
@@ -605,7 +690,8 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) msbfs_kernel(const __grid_co
   const uint64_t gtid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (uint64_t)gridDim.x * blockDim.x;
   if (threadIdx.x < WARPS_PER_BLOCK) sh.bigCnt[threadIdx.x] = 0;
   if (threadIdx.x < 256) sh.perSource[threadIdx.x] = 0;
-  if (threadIdx.x == 0) { sh.acc = 0; sh.updAcc = 0; }
+  if (threadIdx.x == 0) { sh.acc = 0; sh.updAcc = 0; sh.longCnt = 0; }
+  if (threadIdx.x < PULL_LONG_CAP * 8) sh.longAcc[threadIdx.x / 8][threadIdx.x % 8] = 0;
   if (threadIdx.x < 8) sh.liveAcc[threadIdx.x] = 0;
   if (threadIdx.x < WARPS_PER_BLOCK * 7) sh.cnt[threadIdx.x / 7][threadIdx.x % 7] = 0;
   __syncthreads();
