@@ -414,7 +414,7 @@ def closeness_measure(args, torch, blest, rank, world, dist, steps, warmup, want
     whole source set once.  N = 1: one blest_closeness call.  N > 1: rank r runs blest_farness_partial over its source
     range, one all-reduce sums the partial target-side arrays, blest_closeness_from_sums divides."""
     n, rp, ci = load_graph("c5_rmat18", args.shrink, rank, world) if args.config == "c5_rmat18" else gg.make_config("c5_rmat18", args.shrink)
-    g = blest.Graph(n, rp, ci, reorder="none", kappa=args.kappa, ms_pull=not args.no_ms_pull)
+    g = blest.Graph(n, rp, ci, reorder="none", kappa=args.kappa, ms_pull=not args.no_ms_pull, ms_lanes=args.ms_lanes)
     info = g.info()
     stream = torch.cuda.current_stream() if world > 1 else torch.cuda.Stream()
     cc = torch.zeros(n, dtype=torch.float64, device="cuda")
@@ -485,15 +485,16 @@ def closeness_measure(args, torch, blest, rank, world, dist, steps, warmup, want
                        "bvss_bytes": int(info.bvss_bytes),
                        "parallelism": "sources partitioned over ranks + all-reduce of the target-side sums" if world > 1 else "1 GPU",
                        "levels_per_batch": stats["levels"] / max(stats["batches"], 1), "vss_entries_per_step": stats["entries"],
+                       "concurrent_lanes": args.ms_lanes if args.ms_lanes else 8,
                        "pull_levels_per_batch": stats.get("pull_levels", 0) / max(stats["batches"], 1),
                        "pull_neighbours_per_step": stats.get("pull_neighbours", 0),
                        "phase_ms_cta0": {k[:-3]: round(v / 1e6, 2) for k, v in phases.items()}},
             "roofline": {"bound": "l2", "achieved": achieved, "peak": l2_peak, "unit": "GB/s",
                          "frac": (achieved / l2_peak) if achieved else None, "traffic": None,
                          "peak_source": "measured: blest_l2_microbench (48 MB footprint copy, persistent launch configuration)",
-                         "kernel": "msbfs_kernel (persistent cooperative; one launch = all batches)",
+                         "kernel": "msbfs_kernel (persistent cooperative; the batches split over concurrent launches of grid / lanes CTAs)",
                          "algorithmic_bytes_per_launch_mean": float(walg), "ms_per_launch_mean": dev_ms / steps},
-            "gpu_launches": int(steps * (2 if world == 1 else 3)),
+            "gpu_launches": int(steps * ((2 * (args.ms_lanes if args.ms_lanes else 8)) if world == 1 else 3 + 2 * ((args.ms_lanes if args.ms_lanes else 8) - 1))),
         }
         prof = committed_profile(f"c5_rmat18/{args.shrink}/kappa{args.kappa}")
         if prof:
@@ -524,6 +525,7 @@ def main():
     ap.add_argument("--kappa", type=int, default=64)
     ap.add_argument("--tma-tiles", action="store_true", help="options.tune[0]: TMA-staged slice tiles in the balanced phase")
     ap.add_argument("--no-ms-pull", action="store_true", help="options.tune[1]: the multi-source kernel never switches to pull levels")
+    ap.add_argument("--ms-lanes", type=int, default=0, help="options.tune[3]: concurrent lanes of the closeness call (0 = default 8, 1 = one full-grid launch)")
     ap.add_argument("--no-persist", action="store_true", help="options.persist_l2 = off: internal-id levels + gather hand-off")
     ap.add_argument("--keep-trace", action="store_true", help="leave the per-level trace on inside the timed region")
     args = ap.parse_args()

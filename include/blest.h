@@ -103,7 +103,9 @@ typedef struct {
                       instead of 128-bit loads into registers -- measured 14 % slower on config 4, hence off by default
                       (DESIGN.md §6); [1] = 1: the multi-source kernel never switches a batch to pull levels;
                       [2] = 1: the lazy kernel always pre-fills levels_out with -1 (no "level guess");
-                      [3] unused */
+                      [3]: concurrent lanes of the closeness / farness calls (their source batches are split over that
+                      many cooperative launches of grid / lanes CTAs on internal streams, forked from and joined into
+                      the caller's stream): 0 = 8, k = k (1..16; 1 = one launch on the whole grid) */
   int reserved[6]; /* [0]: switching == 5 ("scripted", tests): level l runs bottom-up iff bit min(l,31) is set;
                       [1..5]: tuning overrides of the switch cost model in 0.01 ps per unit (top-down edge, top-down
                       vertex, bottom-up vertex, bottom-up scanned neighbour, bottom-up bitmap word); 0 = default */
@@ -205,13 +207,14 @@ int blest_noalloc_limits(uint32_t *max_srcs, uint64_t *max_state_bytes, uint64_t
 /* Totals of the most recent multi-source launch, for the roofline (needs options.trace): out8[0] work-queue entries
  * (VSS chunks) consumed by Stage 1, [1] quads they hold, [2] slices with a non-zero selection (V_next probed), [3] row words updated
  * by an atomic, [4] dirty slice sets swept by Stage 2, [5] levels (top-down and pull), [6] source batches, [7] neighbours
- * read by the pull levels.  Synchronises the device. */
+ * read by the pull levels; totals over the concurrent lanes of the call.  Synchronises the device. */
 int blest_get_ms_stats(blest_handle_t h, uint64_t *out8);
 /* Where the most recent multi-source launch spent its time (needs options.trace), in nanoseconds of %globaltimer as seen
  * by thread 0 of CTA 0, summed over all batches and levels: out8[0] per-batch init (state clears, source bits, level-0
  * sweep, their barriers), [1] Stage 1 own work, [2] wait at the barrier after Stage 1, [3] Stage 2
  * own work, [4] wait at the barrier after Stage 2, [5] rows a pull level scanned (some live source not
- * there yet), [6] pull levels, [7] 0; a pull level's own work counts under [1], its barrier under [2].  Synchronises the device. */
+ * there yet), [6] pull levels, [7] 0; a pull level's own work counts under [1], its barrier under [2].  With concurrent
+ * lanes the times are those of lane 0 (its share of the batches), the pull counters totals.  Synchronises the device. */
 int blest_get_ms_phases(blest_handle_t h, uint64_t *out8);
 /* Per-level record of the first levels (at most 60, over consecutive batches) of the most recent multi-source launch
  * (needs options.trace): four words per level -- (level << 32 | work-queue entries consumed), ns of Stage 1 + its

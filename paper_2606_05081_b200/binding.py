@@ -158,7 +158,7 @@ def _stream(stream):
 
 def _options(reorder="none", builder=0, validate=False, kernel="auto", switching="auto", contraction="auto", kappa=64,
              trace=True, eta=0.0, gamma=0.0, bu_mask=0, costs=None, persist_l2=True, prune_components=True,
-             queue_capacity=0, tma_tiles=False, ms_pull=True, level_guess=True) -> _Options:
+             queue_capacity=0, tma_tiles=False, ms_pull=True, level_guess=True, ms_lanes=0) -> _Options:
     o = _Options()
     o.reorder = REORDER[reorder] if isinstance(reorder, str) else int(reorder)
     o.builder = int(builder)
@@ -176,6 +176,7 @@ def _options(reorder="none", builder=0, validate=False, kernel="auto", switching
     o.tune[0] = int(bool(tma_tiles))
     o.tune[1] = 0 if ms_pull else 1
     o.tune[2] = 0 if level_guess else 1
+    o.tune[3] = int(ms_lanes)
     o.reserved[0] = int(bu_mask)
     for k, c in enumerate(costs or ()):  # switch cost model overrides, ps per unit (tuning only): td_edge, td_vertex,
         o.reserved[1 + k] = int(round(100 * float(c)))  # bu_vertex, bu_scan, bu_word

@@ -88,6 +88,23 @@ struct blest_graph {
   // pinned staging slots for host `srcs` arrays (consumed before the call returns; recycled once their copy has run)
   struct StageSlot { void* host = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; };
   std::vector<StageSlot> stage;
+  // concurrent lanes of the multi-source calls (launch_ms_lanes): lane 0 is the workspace above on the caller's stream,
+  // lanes 1.. own a stream, an event and a second copy of every per-launch array
+  struct MsLane {
+    cudaStream_t st = nullptr;
+    cudaEvent_t done = nullptr;
+    uint64_t words = 0;  // size of the state arrays (grow-only with kappa, as lane 0)
+    uint32_t *F = nullptr, *F2 = nullptr, *Vc = nullptr, *Vn = nullptr, *live = nullptr;
+    uint8_t* dirty = nullptr;
+    uint2* Q[2] = {nullptr, nullptr};
+    Ctrl* ctrl = nullptr;
+    unsigned long long* farT = nullptr;
+    uint32_t* reachT = nullptr;
+    unsigned long long* stats = nullptr;
+  };
+  std::vector<MsLane> msLanes;   // lanes 1..
+  cudaEvent_t msFork = nullptr;
+  int msLanesUsed = 1;           // lanes of the most recent multi-source launch (blest_get_ms_stats sums over them)
   uint8_t* dDirty = nullptr;
   unsigned long long* dFarT = nullptr;
   uint32_t* dReachT = nullptr;
@@ -263,6 +280,11 @@ void blest_destroy(blest_handle_t h) {
     persist_release(h);
   }
   for (void* p : h->allocs) cudaFree(p);
+  for (auto& ln : h->msLanes) {
+    if (ln.done) cudaEventDestroy(ln.done);
+    if (ln.st) cudaStreamDestroy(ln.st);
+  }
+  if (h->msFork) cudaEventDestroy(h->msFork);
   for (auto& sl : h->stage) {
     if (sl.ev) cudaEventDestroy(sl.ev);
     if (sl.host) cudaFreeHost(sl.host);
@@ -804,6 +826,111 @@ static void fill_ms_params(blest_graph* h, MsParams& p) {
   p.pullMin = (h->opt.tune[1] == 1 || h->directed) ? 0u : std::max(1u, h->Nv / 2u);
 }
 
+// ---- concurrent lanes -------------------------------------------------------------------------------------------------
+// Source batches are independent (PAPER.md:678 partitions them over GPUs); on ONE GPU the persistent kernel does not need
+// the whole grid either: measured on config 5 (kappa = 64), the same launch on 74 of the 148 SMs is only 1.30 x slower and
+// on 37 SMs 1.88 x (57 % of the warp samples of the full-grid launch wait at a grid barrier: small levels, stragglers).
+// Closeness / farness calls therefore split their batches over up to `lanes` cooperative launches of gridMs / lanes CTAs
+// each, on separate streams forked from and joined into the caller's stream by events: while one lane sits in a barrier
+// or a small level, the SMs of the others are busy.  Every lane has its own per-launch arrays; the target-side sums of
+// lanes 1.. are added to lane 0's afterwards.  Cooperative grids are scheduled whole, so the lanes cannot deadlock on each
+// other's barriers.  options.tune[3]: 0 = 8 lanes, k = k lanes (1..16; 1 = the single full-grid launch).
+static int ms_lane_count(const blest_graph* h, uint64_t batches) {
+  int want = h->opt.tune[3] > 0 ? h->opt.tune[3] : 8;
+  want = std::max(1, std::min(want, 16));
+  want = (int)std::min<uint64_t>((uint64_t)want, std::max<uint64_t>(batches, 1));
+  want = std::min(want, std::max(1, h->gridMs));
+  // per-lane workspace: two work queues + four state arrays; keep the extra lanes below 4 GiB in total
+  const uint64_t perLane = (uint64_t)h->qcap * 16u + 4u * h->msWords * 4u + (uint64_t)h->rho * 8u * 12u;
+  while (want > 1 && perLane * (uint64_t)(want - 1) > (4ull << 30)) --want;
+  return want;
+}
+
+static int ensure_ms_lanes(blest_graph* g, int lanes) {
+  int rc;
+  if (!g->msFork) CK(cudaEventCreateWithFlags(&g->msFork, cudaEventDisableTiming));
+  if ((int)g->msLanes.size() < lanes - 1) g->msLanes.resize((size_t)lanes - 1);
+  for (int i = 0; i < lanes - 1; ++i) {
+    blest_graph::MsLane& ln = g->msLanes[(size_t)i];
+    if (!ln.st) CK(cudaStreamCreateWithFlags(&ln.st, cudaStreamNonBlocking));
+    if (!ln.done) CK(cudaEventCreateWithFlags(&ln.done, cudaEventDisableTiming));
+    if (ln.words < g->msWords) {  // (a wider kappa: ensure_ms_workspace has synchronised the device already)
+      for (uint32_t** a : {&ln.F, &ln.F2, &ln.Vc, &ln.Vn}) {
+        if (*a) {
+          auto it = std::find(g->allocs.begin(), g->allocs.end(), (void*)*a);
+          if (it != g->allocs.end()) g->allocs.erase(it);
+          cudaFree(*a);
+          g->wsBytes -= (ln.words * 4 + 15) & ~15ull;
+          *a = nullptr;
+        }
+        if ((rc = dev_alloc(g, a, g->msWords, true))) return rc;
+      }
+      ln.words = g->msWords;
+    }
+    if (!ln.dirty && (rc = dev_alloc(g, &ln.dirty, (uint64_t)g->Ns + 16, true))) return rc;
+    if (!ln.live && (rc = dev_alloc(g, &ln.live, 24, true))) return rc;
+    for (int q = 0; q < 2; ++q)
+      if (!ln.Q[q] && (rc = dev_alloc(g, &ln.Q[q], (uint64_t)g->qcap))) return rc;
+    if (!ln.ctrl && (rc = dev_alloc(g, &ln.ctrl, 1, true))) return rc;
+    if (!ln.farT && (rc = dev_alloc(g, &ln.farT, (uint64_t)g->rho * 8u, true))) return rc;
+    if (!ln.reachT && (rc = dev_alloc(g, &ln.reachT, (uint64_t)g->rho * 8u, true))) return rc;
+    if (!ln.stats && (rc = dev_alloc(g, &ln.stats, MS_STATS_WORDS, true))) return rc;
+  }
+  return BLEST_OK;
+}
+
+// The multi-source kernel over p.nsrcs sources (p = lane 0's arrays, outputs and source range), split over lanes.
+// Enqueues only.  The caller has cleared p.farT / p.reachT / p.farS / p.reachS on `st`.
+static cudaError_t launch_ms_lanes(blest_graph* h, const MsParams& p, cudaStream_t st) {
+  const uint64_t kappa = (uint64_t)p.kappa, batches = (p.nsrcs + kappa - 1) / kappa;
+  int lanes = ms_lane_count(h, batches);
+  if (lanes > 1 && ensure_ms_lanes(h, lanes) != BLEST_OK) {
+    cudaGetLastError();
+    lanes = 1;  // no memory for a second workspace: the single full-grid launch
+  }
+  h->msLanesUsed = lanes;
+  cudaError_t e = cudaSuccess;
+  if (lanes > 1) e = cudaEventRecord(h->msFork, st);
+  const int grid = std::max(1, h->gridMs / lanes);
+  for (int i = 0; i < lanes && e == cudaSuccess; ++i) {
+    const uint64_t b0 = batches * (uint64_t)i / (uint64_t)lanes, b1 = batches * (uint64_t)(i + 1) / (uint64_t)lanes;
+    const uint64_t first = b0 * kappa, end = std::min<uint64_t>(p.nsrcs, b1 * kappa);
+    MsParams q = p;
+    q.srcBase = p.srcBase + first;
+    q.nsrcs = end - first;
+    if (p.srcs) q.srcs = p.srcs + first;
+    if (p.farS) q.farS = p.farS + first;
+    if (p.reachS) q.reachS = p.reachS + first;
+    cudaStream_t s = st;
+    if (i > 0) {
+      blest_graph::MsLane& ln = h->msLanes[(size_t)i - 1];
+      s = ln.st;
+      q.F = ln.F; q.F2 = ln.F2; q.Vc = ln.Vc; q.Vn = ln.Vn; q.live = ln.live; q.dirty = ln.dirty;
+      q.Q[0] = ln.Q[0]; q.Q[1] = ln.Q[1];
+      q.ctrl = ln.ctrl;
+      if (p.stats) q.stats = ln.stats;
+      if (p.farT) q.farT = ln.farT;
+      if (p.reachT) q.reachT = ln.reachT;
+      e = cudaStreamWaitEvent(s, h->msFork, 0);
+      if (e == cudaSuccess && p.farT) e = cudaMemsetAsync(ln.farT, 0, (size_t)h->rho * 8u * 8u, s);
+      if (e == cudaSuccess && p.reachT) e = cudaMemsetAsync(ln.reachT, 0, (size_t)h->rho * 8u * 4u, s);
+    }
+    if (e == cudaSuccess) e = cudaMemsetAsync(q.ctrl, 0, sizeof(Ctrl), s);
+    if (e == cudaSuccess) e = cudaMemsetAsync(i > 0 ? h->msLanes[(size_t)i - 1].stats : h->dMsStats, 0,
+                                              MS_STATS_WORDS * sizeof(unsigned long long), s);
+    if (e == cudaSuccess && q.nsrcs) e = launch_msbfs(q, i == 0 && lanes == 1 ? h->gridMs : grid, s);
+    if (e == cudaSuccess && i > 0) e = cudaEventRecord(h->msLanes[(size_t)i - 1].done, s);
+  }
+  for (int i = 1; i < lanes && e == cudaSuccess; ++i) {
+    blest_graph::MsLane& ln = h->msLanes[(size_t)i - 1];
+    e = cudaStreamWaitEvent(st, ln.done, 0);
+    if (e == cudaSuccess && (p.farT || p.reachT))
+      e = launch_add_partial_sums(p.farT, p.reachT, p.farT ? ln.farT : nullptr, p.reachT ? ln.reachT : nullptr,
+                                  (uint64_t)h->rho * 8u, st);
+  }
+  return e;
+}
+
 // Stream-ordered temporaries of one multi-source call: device buffers from the stream's memory pool
 // (cudaMallocAsync / cudaFreeAsync: no host block), the caller's `srcs` copied through a pinned staging slot.
 struct MsTemps {
@@ -881,6 +1008,7 @@ int blest_msbfs(blest_handle_t h, const uint32_t* srcs, uint32_t k, int32_t* lev
   h->lastCtrl = h->dCtrl;
   if (e == cudaSuccess) e = cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st);
   if (e == cudaSuccess) e = cudaMemsetAsync(h->dMsStats, 0, MS_STATS_WORDS * sizeof(unsigned long long), st);
+  h->msLanesUsed = 1;
   if (e == cudaSuccess) e = launch_msbfs(p, h->gridMs, st);
   if (e == cudaSuccess && !devOut)
     e = cudaMemcpyAsync(levels_out, dLevels, (size_t)k * h->n * 4, cudaMemcpyDeviceToHost, st);
@@ -934,9 +1062,7 @@ static int closeness_impl(blest_handle_t h, const uint32_t* srcs, uint64_t n_src
   if (e == cudaSuccess && farOut && !farDev) e = tmp.alloc((void**)&dFarO, n_srcs * 8);
   if (e == cudaSuccess && reachOut && !reachDev) e = tmp.alloc((void**)&dReachO, n_srcs * 4);
   h->lastCtrl = h->dCtrl;
-  if (e == cudaSuccess) e = cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st);
-  if (e == cudaSuccess) e = cudaMemsetAsync(h->dMsStats, 0, MS_STATS_WORDS * sizeof(unsigned long long), st);
-  if (e == cudaSuccess) e = launch_msbfs(p, h->gridMs, st);
+  if (e == cudaSuccess) e = launch_ms_lanes(h, p, st);
   if (e == cudaSuccess)
     e = launch_closeness_finalize(h->n, h->rho, h->hasPerm ? h->dPerm : nullptr, p.farT, p.reachT, p.farS, p.reachS, n_srcs,
                                   cc ? (ccDev ? cc : dCc) : nullptr,
@@ -970,9 +1096,7 @@ int blest_farness_partial(blest_handle_t h, uint32_t first, uint32_t count, uint
   h->lastCtrl = h->dCtrl;
   cudaError_t e = cudaMemsetAsync(h->dFarT, 0, (size_t)h->rho * 8u * 8u, st);
   if (e == cudaSuccess) e = cudaMemsetAsync(h->dReachT, 0, (size_t)h->rho * 8u * 4u, st);
-  if (e == cudaSuccess) e = cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st);
-  if (e == cudaSuccess) e = cudaMemsetAsync(h->dMsStats, 0, MS_STATS_WORDS * sizeof(unsigned long long), st);
-  if (e == cudaSuccess) e = launch_msbfs(p, h->gridMs, st);
+  if (e == cudaSuccess) e = launch_ms_lanes(h, p, st);
   // target-side sums in ORIGINAL vertex ids (the finalize kernel maps id -> getVI(perm[id]))
   if (e == cudaSuccess)
     e = launch_closeness_finalize(h->n, h->rho, h->hasPerm ? h->dPerm : nullptr, p.farT, p.reachT, nullptr, nullptr, h->n,
@@ -1005,6 +1129,7 @@ int blest_closeness_noalloc(blest_handle_t h, const uint32_t* srcs_dev, uint32_t
   fill_ms_params(h, p);  // graph arrays, work queues and control block of the handle: allocated by blest_build
   h->lastCtrl = h->dCtrl;
   cudaError_t e = cudaMemsetAsync(h->dCtrl, 0, sizeof(Ctrl), st);
+  h->msLanesUsed = 1;
   if (e == cudaSuccess) e = launch_closeness_noalloc(p, srcs_dev, n_srcs, h->gridMs, out_dev, st);
   if (e != cudaSuccess) return ms_fail(e);
   return BLEST_OK;
@@ -1024,6 +1149,11 @@ int blest_get_ms_stats(blest_handle_t h, uint64_t* out8) {
   if (!h->dMsStats) return BLEST_OK;
   CK(cudaDeviceSynchronize());
   CK(cudaMemcpy(out8, h->dMsStats, 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+  for (int i = 1; i < h->msLanesUsed && (size_t)i - 1 < h->msLanes.size(); ++i) {  // totals over the lanes of the launch
+    uint64_t t[8];
+    CK(cudaMemcpy(t, h->msLanes[(size_t)i - 1].stats, 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+    for (int k = 0; k < 8; ++k) out8[k] += t[k];
+  }
   return BLEST_OK;
 }
 
@@ -1034,6 +1164,12 @@ int blest_get_ms_phases(blest_handle_t h, uint64_t* out8) {
   if (!h->dMsStats) return BLEST_OK;
   CK(cudaDeviceSynchronize());
   CK(cudaMemcpy(out8, h->dMsStats + 8, 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+  for (int i = 1; i < h->msLanesUsed && (size_t)i - 1 < h->msLanes.size(); ++i) {  // times: lane 0's; pull counters: totals
+    uint64_t t[8];
+    CK(cudaMemcpy(t, h->msLanes[(size_t)i - 1].stats + 8, 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+    out8[5] += t[5];
+    out8[6] += t[6];
+  }
   return BLEST_OK;
 }
 

@@ -115,6 +115,8 @@ cudaError_t launch_bfs_lazy(const BfsParams& p, int gridBlocks, cudaStream_t st,
                             float hitRatio);
 cudaError_t launch_bfs_eager(const BfsParams& p, int gridBlocks, cudaStream_t st);
 cudaError_t launch_isolated_source(int32_t* out, uint32_t n, uint32_t src, cudaStream_t st);
+cudaError_t launch_add_partial_sums(unsigned long long* far0, uint32_t* reach0, const unsigned long long* far1,
+                                    const uint32_t* reach1, uint64_t count, cudaStream_t st);
 cudaError_t launch_msbfs(const MsParams& p, int gridBlocks, cudaStream_t st);
 cudaError_t launch_closeness_finalize(uint32_t n, uint32_t rho, const uint32_t* perm, const unsigned long long* farT,
                                       const uint32_t* reachT, const unsigned long long* farS, const uint32_t* reachS,

@@ -873,6 +873,24 @@ cudaError_t launch_msbfs(const MsParams& p, int gridBlocks, cudaStream_t st) {
   return cudaLaunchCooperativeKernel(k, dim3(gridBlocks), dim3(BLOCK_THREADS), args, sizeof(MsShared), st);
 }
 
+// far0 += far1, reach0 += reach1 (the target-side sums of a concurrent lane, api.cu launch_ms_lanes)
+namespace {
+__global__ void add_partial_sums_kernel(unsigned long long* far0, uint32_t* reach0, const unsigned long long* far1,
+                                        const uint32_t* reach1, uint64_t count) {
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += (uint64_t)gridDim.x * blockDim.x) {
+    if (far0 && far1) far0[i] += far1[i];
+    if (reach0 && reach1) reach0[i] += reach1[i];
+  }
+}
+}  // namespace
+cudaError_t launch_add_partial_sums(unsigned long long* far0, uint32_t* reach0, const unsigned long long* far1,
+                                    const uint32_t* reach1, uint64_t count, cudaStream_t st) {
+  const int threads = 256;
+  const int blocks = (int)std::min<uint64_t>((count + threads - 1) / threads, 148ull * 8);
+  add_partial_sums_kernel<<<blocks > 0 ? blocks : 1, threads, 0, st>>>(far0, reach0, far1, reach1, count);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_closeness_finalize(uint32_t n, uint32_t rho, const uint32_t* perm, const unsigned long long* farT,
                                       const uint32_t* reachT, const unsigned long long* farS, const uint32_t* reachS,
                                       uint64_t nsrcs, double* cc, unsigned long long* farOut, uint32_t* reachOut,

@@ -453,6 +453,45 @@ def test_level_guess(blest, torch_cuda, reorder):
         assert (used > 0) == guess
 
 
+@pytest.mark.parametrize("lanes", [1, 2, 3, 8, 16])
+def test_ms_concurrent_lanes(blest, torch_cuda, lanes):
+    """Closeness / farness calls split their source batches over concurrent cooperative launches (options.tune[3]):
+    every lane count gives the oracle's farness / reach / closeness, for all vertices (target-side sums added over the
+    lanes), for a source subset (per-source sums, disjoint per lane) and for a source range; the launch totals are sums
+    over the lanes."""
+    torch = torch_cuda
+    n, rp, ci = gg.disjoint_union(gg.rmat(10, 10, 31), gg.grid2d(9, 11), gg.star(40, 1), gg.empty(6))
+    far_w, reach_w, cc_w, _ = oracle.closeness(n, rp, ci)
+    for kappa, reorder in ((32, "none"), (64, "degree"), (128, "none")):
+        with blest.Graph(n, rp, ci, kappa=kappa, reorder=reorder, ms_lanes=lanes) as g:
+            far = torch.zeros(n, dtype=torch.int64, device="cuda")
+            reach = torch.zeros(n, dtype=torch.int32, device="cuda")
+            cc = torch.zeros(n, dtype=torch.float64, device="cuda")
+            for _ in range(2):  # twice: the lanes' workspaces are reused
+                g.farness(far, reach)
+                g.closeness(cc)
+                assert np.array_equal(far.cpu().numpy().view(np.uint64), far_w)
+                assert np.array_equal(reach.cpu().numpy().view(np.uint32), reach_w)
+                assert np.array_equal(cc.cpu().numpy(), cc_w)
+            st = g.ms_stats()
+            assert st["batches"] == -(-n // kappa) and st["levels"] >= st["batches"]
+            sub = np.concatenate([np.arange(5, n, 7), [0, n - 1, 5]]).astype(np.uint32)
+            f2, r2 = np.zeros(sub.size, dtype=np.uint64), np.zeros(sub.size, dtype=np.uint32)
+            g.farness(f2, r2, srcs=sub)
+            assert np.array_equal(f2, far_w[sub]) and np.array_equal(r2, reach_w[sub])
+            assert g.ms_stats()["batches"] == -(-sub.size // kappa)
+            pf = torch.zeros(n, dtype=torch.int64, device="cuda")
+            pr = torch.zeros(n, dtype=torch.int32, device="cuda")
+            tot_f, tot_r = torch.zeros_like(pf), torch.zeros_like(pr)
+            for first, count in ((0, 333), (333, n - 333)):
+                g.farness_partial(first, count, pf, pr)
+                tot_f += pf
+                tot_r += pr
+            assert np.array_equal(tot_f.cpu().numpy().view(np.uint64), far_w)
+            assert np.array_equal(tot_r.cpu().numpy().view(np.uint32), reach_w)
+            assert g.last_status() == 0
+
+
 @pytest.mark.parametrize("kappa", [32, 64, 128, 256])
 def test_msbfs_pull_levels(blest, torch_cuda, kappa):
     """The pull levels of the multi-source kernel (a batch switches once a level's queue holds half of all VSSs): farness /
