@@ -44,6 +44,7 @@ struct LazyShared {
   uint32_t wlCnt;
   uint32_t wlBase;
   uint32_t buDecision;  // direction of the level, evaluated by the thread that read the control words
+  unsigned long long degVisited;  // (thread 0) degree sum of the vertices visited so far: the switch's `mu`
   uint32_t guess;       // the level levels_out is pre-filled with (0 = none; see the kernel)
   uint32_t guessSlot;   // degree class of the source
   uint32_t bestLevel;   // (thread 0) the level that discovered the most vertices so far, and how many
@@ -70,13 +71,18 @@ struct LazyShared {
   uint32_t hub[HUB_BITS / 32];  // top-down Stage 1: low-id vertices this CTA has already marked in this level
 };
 
+// Per-LANE counters of one level: 32 bits each (a lane's share of a level is far below 2^32 vertices, edge endpoints or
+// bytes; nnz < 2^32 bounds the degree sum), widened when the warp's values are added up -- five 64-bit counters per thread
+// cost the persistent kernel ten of its 64 registers.  `unv` is signed: discoveries are subtracted from it.
 struct Counters {
-  unsigned long long nnew = 0, unv = 0, mf = 0, scanned = 0, qbytes = 0;
+  uint32_t nnew = 0;
+  int32_t unv = 0;
+  uint32_t mf = 0, scanned = 0, qbytes = 0;
 };
 
 // warp shuffle reduce -> shared atomics -> one global atomic per block and counter
 __device__ __forceinline__ void block_accumulate(LazyShared& sh, const Counters& c, Ctrl* ctrl, uint32_t ci) {
-  unsigned long long v[5] = {c.nnew, c.unv, c.mf, c.scanned, c.qbytes};
+  unsigned long long v[5] = {c.nnew, (unsigned long long)(long long)c.unv, c.mf, c.scanned, c.qbytes};
 #pragma unroll
   for (int k = 0; k < 5; ++k) {
 #pragma unroll
@@ -385,7 +391,7 @@ __device__ __forceinline__ void td_phase_a(const BfsParams& p, LazyShared& sh, c
           const uint32_t s = t * 4u + k;
           a[k] = __ldg(&p.setPtr[s]);
           nq[k] = __ldg(&p.setPtr[s + 1]) - a[k];
-          c.qbytes += 20ull * nq[k] + 8ull;
+          c.qbytes += 20u * nq[k] + 8u;
         }
       }
 #pragma unroll
@@ -415,13 +421,13 @@ __device__ __forceinline__ void td_phase_a(const BfsParams& p, LazyShared& sh, c
           ebits &= ebits - 1;
           r0[q] = __ldg(&p.rowptr[u]);
           deg[q] = __ldg(&p.rowptr[u + 1]) - r0[q];
-          c.qbytes += 8ull;
+          c.qbytes += 8u;
         }
       }
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         if (!__any_sync(FULL, deg[q] != 0)) continue;
-        c.qbytes += 4ull * deg[q];
+        c.qbytes += 4u * deg[q];
         uint32_t big = __ballot_sync(FULL, deg[q] > bigEdges);
         while (big) {
           const int src = __ffs(big) - 1;
@@ -774,7 +780,7 @@ __device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_
       tag = slotTag[lane];
       ptr = __ldg(&p.rowptrIn[uu]) + 2u;
       e = __ldg(&p.rowptrIn[uu + 1]);
-      c.qbytes += 8ull;
+      c.qbytes += 8u;
     }
     bool f = false;
     const uint32_t stop = min(e, ptr + SERIAL_CAP);
@@ -790,7 +796,7 @@ __device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_
       for (int j = 0; j < 4; ++j)
         if ((uint32_t)j < cnt && ((fwd[j] >> (v[j] & 31u)) & 1u)) f = true;
       c.scanned += cnt;
-      c.qbytes += 4ull * cnt;
+      c.qbytes += 4u * cnt;
       ptr += cnt;
     }
     // long lists are finished by the whole warp
@@ -807,7 +813,7 @@ __device__ __forceinline__ uint32_t bu_resolve(const BfsParams& p, const uint32_
           const uint32_t v = __ldg(&p.colidxIn[idx]);
           hit = (Fp[v >> 5] >> (v & 31u)) & 1u;
           ++c.scanned;
-          c.qbytes += 4ull;
+          c.qbytes += 4u;
         }
         if (__ballot_sync(FULL, hit)) { ff = true; break; }
       }
@@ -1102,7 +1108,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     p.lvl[p.srcLvl] = 0;  // L[src] = 0 (after the fill: ordered by the barrier)
   }
 
-  unsigned long long degVisited = 0;  // sum of degrees of all visited vertices
+  if (threadIdx.x == 0) sh.degVisited = 0;  // sum of degrees of all visited vertices (only the deciding thread needs it)
   uint32_t level = 1;
   for (;; ++level) {
     const uint32_t cp = (level - 1) % 3u, ci = level % 3u, cn = (level + 1) % 3u;
@@ -1113,7 +1119,8 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       sh.ctl[2] = ld_volatile(&ctrl->unvisited[cp]);
       sh.ctl[3] = ld_volatile(&ctrl->wlc[cp]);
       // the switch (a powf and an expf) is evaluated once per CTA, not by every warp
-      const unsigned long long dv = degVisited + sh.ctl[1];
+      const unsigned long long dv = sh.degVisited + sh.ctl[1];
+      if (sh.ctl[0] != 0 && sh.ctl[2] != 0) sh.degVisited = dv;  // (the level runs: its frontier joins the visited set)
       sh.buDecision = choose_bottom_up(p, level, sh.ctl[0], sh.ctl[1], sh.ctl[2], p.nnz > dv ? p.nnz - dv : 0ull) ? 1u : 0u;
       // the level that discovered the most vertices so far: the next call's guess (kept in shared memory: no registers)
       if (level >= 2u && sh.ctl[0] > sh.bestCount) { sh.bestCount = sh.ctl[0]; sh.bestLevel = level - 1u; }
@@ -1128,7 +1135,6 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     const bool storeLv = level != sh.guess;  // the pre-fill already holds this level
     if (nf == 0) break;  // empty frontier ("terminates at the first level with x = 0")
     if (unvAll == 0) break;  // nothing left that could be discovered (everything outside the component is pre-marked)
-    degVisited += mf;
     const unsigned long long nu = unvAll;  // zero-degree vertices count as visited from the start
     const uint32_t* Fp = p.F[cp];
     uint32_t* Fn = p.F[ci];
@@ -1171,10 +1177,10 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
         c.nnew += disc ? 1u : 0u;
         wl_append(sh, p.WL[1], &ctrl->wlc[ci], v >> 5, disc && old == 0u, lane);
       }
-      c.unv = 0ull - c.nnew;
+      c.unv = -(int32_t)c.nnew;
       if (gwarp == 0 && lane == 0) {
-        c.unv += unvAll;
-        c.qbytes += 8ull + 4ull * srcDeg;
+        c.unv += (int32_t)unvAll;
+        c.qbytes += 8u + 4u * srcDeg;
       }
       wl_flush(sh, p.WL[1], &ctrl->wlc[ci]);
       block_accumulate(sh, c, ctrl, ci);
