@@ -44,6 +44,8 @@ struct LazyShared {
   uint32_t wlCnt;
   uint32_t wlBase;
   uint32_t buDecision;  // direction of the level, evaluated by the thread that read the control words
+  unsigned long long tStage1;     // (leader) %globaltimer after the level's Stage-1 barrier
+  unsigned int epoch;             // (thread 0) grid barriers executed on this control block
   unsigned long long degVisited;  // (thread 0) degree sum of the vertices visited so far: the switch's `mu`
   uint32_t guess;       // the level levels_out is pre-filled with (0 = none; see the kernel)
   uint32_t guessSlot;   // degree class of the source
@@ -1006,9 +1008,8 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
   // The control block is never memset between calls: the barrier counter is monotone over the launches on this
   // handle (stream-ordered), `epochBase` is where the previous launch left it, and the leader resets the per-call
   // fields below.  Only thread 0 of a CTA evaluates the barrier target, so only it needs the true epoch.
-  unsigned int epoch = 0;
   if (threadIdx.x == 0) {
-    epoch = ld_volatile(&ctrl->epochBase);
+    sh.epoch = ld_volatile(&ctrl->epochBase);
     // LEVEL GUESS.  On a low-diameter graph one level discovers most of the component (config 4: level 3 finds 8.8 M of the
     // 11 M reachable vertices), and its scattered level writes + original-id loads are a third of that level's time.
     // The previous call on this handle (from a source of similar degree) left the level that discovered the most vertices in
@@ -1102,7 +1103,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
     // (the source is not counted twice when it is itself pre-marked: a directed graph's source of in-degree 0)
     ctrl->unvisited[0] = (unsigned long long)min((uint64_t)p.n, (uint64_t)nSW * 32u) - (p.srcPremarked ? 0u : 1u) - p.nIsoInSweep;
   }
-  grid_barrier(&ctrl->bar, epoch);
+  grid_barrier_sh(&ctrl->bar, &sh.epoch);
   if (leader) {
     ctrl->tInit = globaltimer() - ctrl->t0;
     p.lvl[p.srcLvl] = 0;  // L[src] = 0 (after the fill: ordered by the barrier)
@@ -1149,7 +1150,6 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       ctrl->nBig[cn] = 0;
       ctrl->qc[cn] = 0;
     }
-    unsigned long long tStage1 = 0;
     if (level == 1 && !bottomUp && p.switching == 0) {
       // Level 1 needs no probe, no filter and no sweep: the neighbours of the source other than itself are all unvisited,
       // so each edge of the source finalises its target on the spot (one phase, one barrier instead of two and a sweep);
@@ -1184,12 +1184,12 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       }
       wl_flush(sh, p.WL[1], &ctrl->wlc[ci]);
       block_accumulate(sh, c, ctrl, ci);
-      grid_barrier(&ctrl->bar, epoch);
-      if (leader) tStage1 = globaltimer();
+      grid_barrier_sh(&ctrl->bar, &sh.epoch);
+      if (leader) sh.tStage1 = globaltimer();
     } else if (bottomUp) {
       bu_level(p, sh, level, Fp, Fn, Fs, p.WL[level & 1u], ctrl, ci, nu, storeLv);
-      grid_barrier(&ctrl->bar, epoch);
-      if (leader) tStage1 = globaltimer();
+      grid_barrier_sh(&ctrl->bar, &sh.epoch);
+      if (leader) sh.tStage1 = globaltimer();
     } else {
       const Marks mk{p.V, Fn, p.hubFilter || mf > 4ull * nu, sh.hub, p.hubFilter ? HUB_BITS : 0u, p.n};
       if (p.hubFilter) {
@@ -1197,18 +1197,18 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
         __syncthreads();
       }
       td_phase_a<CONTR>(p, sh, p.WL[(level - 1) & 1u], wlCount, Fp, mk, ctrl, ci);
-      grid_barrier(&ctrl->bar, epoch);
+      grid_barrier_sh(&ctrl->bar, &sh.epoch);
       if (threadIdx.x == 0) sh.ctl[0] = ld_volatile(&ctrl->qc[ci]);
       __syncthreads();
       const uint32_t nChunks = (uint32_t)sh.ctl[0];
       __syncthreads();
       if (nChunks) {  // hubs: equal chunks spread over the grid
         td_phase_b<CONTR>(p, sh, min(nChunks, p.chunkCap), mk);
-        grid_barrier(&ctrl->bar, epoch);
+        grid_barrier_sh(&ctrl->bar, &sh.epoch);
       }
-      if (leader) tStage1 = globaltimer();
+      if (leader) sh.tStage1 = globaltimer();
       td_finalize(p, sh, level, Fn, Fs, p.WL[level & 1u], ctrl, ci, storeLv);
-      grid_barrier(&ctrl->bar, epoch);
+      grid_barrier_sh(&ctrl->bar, &sh.epoch);
     }
     if (leader && p.trace && level - 1 < p.traceCap) {
       blest_level_trace_t r;
@@ -1222,14 +1222,14 @@ __global__ void __launch_bounds__(BLOCK_THREADS, 1) bfs_lazy_kernel(const __grid
       r.unvisited = (uint32_t)(ua + p.nIsoInSweep + ((unsigned long long)p.n - min((uint64_t)p.n, (uint64_t)nSW * 32u)));
       r.reserved = (bottomUp ? 0u : ld_volatile(&ctrl->nBig[ci])) | (storeLv ? 0u : 0x80000000u);
       r.t_ns = globaltimer() - ctrl->t0;
-      r.t_stage1_ns = tStage1 - ctrl->t0;
+      r.t_stage1_ns = sh.tStage1 - ctrl->t0;
       p.trace[level - 1] = r;
     }
   }
   if (leader) {
     ctrl->nlevels = level - 1;
     ctrl->guess[sh.guessSlot] = sh.bestLevel;
-    ctrl->epochBase = epoch;  // every CTA has executed the same barriers: the next launch continues from here
+    ctrl->epochBase = sh.epoch;  // every CTA has executed the same barriers: the next launch continues from here
   }
 
   // A10 as a separate pass (p.gather): the levels were written in internal ids (coalesced, no iperm read) and go to

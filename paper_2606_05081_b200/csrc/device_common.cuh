@@ -110,6 +110,23 @@ __device__ __forceinline__ void grid_barrier(unsigned int* bar, unsigned int& ep
   __syncthreads();
 }
 
+// The same barrier with the epoch kept in a shared-memory word that only thread 0 touches (no register of the other
+// threads): the lazy kernel sits at its register limit.
+__device__ __forceinline__ void grid_barrier_sh(unsigned int* bar, unsigned int* epochSlot) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const unsigned int epoch = *epochSlot + 1u;
+    *epochSlot = epoch;
+    const unsigned int target = epoch * gridDim.x;
+    asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(bar) : "memory");
+    unsigned int v;
+    do {
+      asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+    } while ((int)(v - target) < 0);
+  }
+  __syncthreads();
+}
+
 // Same barrier on the {bar, tail} word: returns the queue tail as it stands once every CTA has arrived (each CTA's
 // appends precede its arrival, so the value is final).  `slot` is a shared-memory word for the broadcast.
 __device__ __forceinline__ unsigned int grid_barrier_tail(unsigned int* bar, unsigned int& epoch, unsigned int* slot) {
